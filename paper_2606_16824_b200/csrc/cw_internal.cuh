@@ -1,0 +1,263 @@
+// Internal definitions shared by the CUDA translation units of libcachewise.so (sm_100a only).
+// Nothing here is shared with oracle/ (the CPU checker): constants are restated from DESIGN.md R1-R5.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/cachewise.h"
+
+typedef uint64_t u64;
+typedef uint32_t u32;
+typedef int32_t i32;
+
+// ---- latched device status bits (cw_sync translates them) --------------------------------------------
+#define CWS_INVAL 1u
+#define CWS_CAPACITY 2u
+
+// ---- stage 1 constants (R1) -------------------------------------------------------------
+#define CW_A 0x9E3779B97F4A7C15ull
+#define CW_K2 0x6A09E667F3BCC909ull
+#define CW_K3 0xBB67AE8584CAA73Bull
+#define CW_K5 0x3C6EF372FE94F82Bull
+#define CW_K7 0xA54FF53A5F1D36F1ull
+#define CW_K11 0x510E527FADE682D1ull
+
+__host__ __device__ constexpr u64 cw_fin(u64 x) {
+    x ^= x >> 32;
+    x *= CW_K2;
+    x ^= x >> 29;
+    x *= CW_K3;
+    x ^= x >> 32;
+    return x;
+}
+__host__ __device__ constexpr u64 cw_pow(u64 base, u64 e) {
+    u64 r = 1;
+    while (e) {
+        if (e & 1) r *= base;
+        base *= base;
+        e >>= 1;
+    }
+    return r;
+}
+
+// ---- table (R2): open addressing, linear probing, 16-byte slots -----------------------------
+struct __align__(16) cw_slot {
+    u64 key;  // 0 = EMPTY, 2^64-1 = TOMBSTONE
+    u32 loc;
+    u32 idx;  // 0xFFFFFFFF except inside an insert batch (lowest input index of the key)
+};
+#define CW_KEY_EMPTY 0ull
+#define CW_KEY_TOMB 0xFFFFFFFFFFFFFFFFull
+#define CW_LOC_PENDING 0xFFFFFFFEu
+
+__host__ __device__ __forceinline__ u64 cw_remap_key(u64 k) {
+    if (k == CW_KEY_EMPTY) return 1ull;
+    if (k == CW_KEY_TOMB) return CW_KEY_TOMB - 1;
+    return k;
+}
+
+// ---- stage 1 launch geometry ---------------------------------------------------------------------------
+#define CWH_WARPS 8                   // consumer warps per CTA
+#define CWH_UNIT (32 * CWH_WARPS)     // blocks per unit (one unit = one CTA iteration)
+#define CWH_UNIT_LOG2 8
+#define CWH_STAGES 3                  // smem ring depth
+#define CWH_STAGE_BYTES (CWH_UNIT * 64 + 16)
+
+struct cw_hash_ctl {  // device-resident, self-cleaning (last CTA resets ticket/done and bumps epoch)
+    u32 ticket;
+    u32 done;
+    u32 epoch;
+    u32 pad;
+};
+
+// ---- stage 3 scratch -------------------------------------------------------------------------------
+#define CWE_BINS 2048          // 11-bit digits
+#define CWE_DIGIT_BITS 11
+#define CWE_PASSES 9           // ceil(96/11): 64-bit score then 32-bit id
+#define CWE_SMALL 4096         // finish in one CTA when the candidate set is this small
+#define CWE_SORT_RUN 4096      // victims sorted in runs of this size, then rank-merged
+
+struct cw_evict_state {
+    u32 n_evictable;   // candidates appended by the score kernel
+    u32 want;          // min(deficit, cap, n_evictable)
+    u32 remaining;     // victims still to be taken from the current candidate set
+    u32 n_cand[2];     // candidate counts of the ping-pong buffers
+    u32 n_out;         // victims emitted so far (unsorted)
+    u32 done;          // selection finished
+    u32 pass;          // next digit index
+    u32 thr_digit;     // threshold digit of the current pass
+    u32 cur;           // which candidate buffer is current
+    u32 pad[6];
+};
+
+struct cw_ctx {
+    cw_config cfg;
+    cudaStream_t s_main, s_copy;
+    bool own_copy_stream;
+    u64 page_bytes;
+    // table
+    cw_slot* table;
+    u64 n_slots;
+    u32* ins_slot;   // scratch: slot index per input of an insert batch
+    u32 ins_cap;
+    // metadata SoA, per tier
+    u32* meta_session[2];
+    u32* meta_last_access[2];
+    u32* meta_depth[2];
+    u32* meta_ref_flags[2];
+    u32 tier_size[2];
+    // status
+    u32* d_status;
+    u32* h_status;  // pinned
+    // stage 1
+    cw_hash_ctl* hash_ctl;
+    u64* hash_agg;
+    u32* hash_flag;
+    u64 hash_slots;
+    int hash_grid;
+    // stage 2a
+    u32* m_first_miss;
+    u32* m_max_hit;
+    u32* m_host_hits;
+    // stage 3
+    u32* tau_q;
+    u64* cand_score[2];
+    u32* cand_id[2];
+    u64* out_score;
+    u32* out_id;
+    u32* hist;  // CWE_PASSES * CWE_BINS
+    cw_evict_state* ev;
+    u32 ev_cap;
+    // stage 4
+    uint8_t* staging;
+    cudaEvent_t ev_gather[2], ev_copy[2], ev_join;
+    int copy_grid;
+    int n_sm;
+    u64 launches;
+    char err[256];
+};
+
+#define CW_CUDA(ctx, call)                                                                              \
+    do {                                                                                                \
+        cudaError_t e__ = (call);                                                                       \
+        if (e__ != cudaSuccess) {                                                                       \
+            snprintf((ctx)->err, sizeof((ctx)->err), "%s:%d %s: %s", __FILE__, __LINE__, #call,         \
+                     cudaGetErrorString(e__));                                                          \
+            return CW_E_CUDA;                                                                           \
+        }                                                                                               \
+    } while (0)
+
+#define CW_LAUNCH_CHECK(ctx)                                                                            \
+    do {                                                                                                \
+        (ctx)->launches++;                                                                              \
+        cudaError_t e__ = cudaGetLastError();                                                           \
+        if (e__ != cudaSuccess) {                                                                       \
+            snprintf((ctx)->err, sizeof((ctx)->err), "%s:%d launch: %s", __FILE__, __LINE__,            \
+                     cudaGetErrorString(e__));                                                          \
+            return CW_E_CUDA;                                                                           \
+        }                                                                                               \
+    } while (0)
+
+static inline bool cw_aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
+// ---- small device helpers ------------------------------------------------------------------------------
+__device__ __forceinline__ u64 shfl64(u64 v, int src) {
+    u32 lo = __shfl_sync(0xffffffffu, (u32)v, src);
+    u32 hi = __shfl_sync(0xffffffffu, (u32)(v >> 32), src);
+    return ((u64)hi << 32) | lo;
+}
+__device__ __forceinline__ u64 shfl64_xor(u64 v, int m) {
+    u32 lo = __shfl_xor_sync(0xffffffffu, (u32)v, m);
+    u32 hi = __shfl_xor_sync(0xffffffffu, (u32)(v >> 32), m);
+    return ((u64)hi << 32) | lo;
+}
+__device__ __forceinline__ u64 shfl64_up(u64 v, int d) {
+    u32 lo = __shfl_up_sync(0xffffffffu, (u32)v, d);
+    u32 hi = __shfl_up_sync(0xffffffffu, (u32)(v >> 32), d);
+    return ((u64)hi << 32) | lo;
+}
+__device__ __forceinline__ u32 smem_u32(const void* p) { return (u32)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(u32 bar, u32 count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(u32 bar, u32 bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(u32 bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(u32 bar, u32 parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+// TMA 1-D bulk copy global -> shared, completion on an mbarrier, L2 evict-first hint for streamed inputs
+__device__ __forceinline__ void bulk_g2s(u32 dst, const void* src, u32 bytes, u32 bar, u64 policy) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
+        "l"(src), "r"(bytes), "r"(bar), "l"(policy)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s_plain(u32 dst, const void* src, u32 bytes, u32 bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* dst, u32 src, u32 bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() {
+    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+template <int N>
+__device__ __forceinline__ void bulk_wait_all() {
+    asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ u64 policy_evict_first() {
+    u64 p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ u32 ld_acquire_u32(const u32* p) {
+    u32 v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_u32(u32* p, u32 v) {
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ u64 ld_relaxed_u64(const u64* p) {
+    u64 v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// per-TU entry points (host side), called from cw_api.cu
+int32_t cwi_hash_blocks(cw_ctx*, const i32*, const u64*, const u32*, const u64*, const u64*, const u64*, u32, u64*);
+int32_t cwi_match_prefix(cw_ctx*, const u64*, const u64*, u32, u32*, u32*, u32*);
+int32_t cwi_table_insert(cw_ctx*, const u64*, const u32*, u32, u32*);
+int32_t cwi_table_erase(cw_ctx*, const u64*, u32);
+int32_t cwi_table_retag(cw_ctx*, const u64*, const u32*, u32);
+int32_t cwi_table_lookup(cw_ctx*, const u64*, u32, u32*);
+int32_t cwi_schedule(cw_ctx*, u32, const u32*, const u32*, const u64*, const u32*, u32, u32, u32, u32, u32*, u32*,
+                     u32*);
+int32_t cwi_score_evict(cw_ctx*, u32, u32, u32, const uint8_t*, const int16_t*, i32, const uint8_t*, const u32*,
+                        const u32*, u32, u32*, u64*, u32*, u32);
+int32_t cwi_copy_pages(cw_ctx*, cudaStream_t, const u32* d_ids, const u32* d_num, u32 first, u32 cap, void* d_staged,
+                       bool gather);
+int32_t cwi_blocks_update(cw_ctx*, u32, const u32*, u32, const u32*, const u32*, const u32*, const u32*);
+int cwi_hash_grid(int n_sm);
+int cwi_copy_grid(int n_sm);

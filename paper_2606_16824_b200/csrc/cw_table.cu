@@ -1,0 +1,328 @@
+// Stage 2a — resident-block table and prefix match (cw_match_prefix, cw_table_*).  DESIGN.md R2.
+//
+// Table: 2^t slots of 16 bytes {key u64, loc u32, idx u32}, linear probing from slot (key & mask).  Two
+// slots share a 32-byte sector, eight a 128-byte line, so a probe sequence walks one line before it
+// touches the next ("coalesced buckets").  Lookups are wait-free reads (one LDG.128 per slot).
+//
+// Insert is lock-free and DETERMINISTIC (result independent of CAS order):
+//   pass 1  walk to the key or to the end of the cluster; claim the first reusable slot with a 64-bit CAS on
+//           the key; every thread of the same key then atomicMin's its input index into slot.idx
+//   pass 2  slot.loc == PENDING  <=> the key was claimed in this batch: input idx wins and writes its loc;
+//           every input reports the surviving loc
+//   pass 3  the winners restore slot.idx = 0xFFFFFFFF
+// (All same-key threads follow one probe sequence whose slots only go from reusable to occupied during the
+// batch, so they converge on the same slot.)
+//
+// Match: one lane per hash, flat over hashes[]; a warp finds its request by a 32-ary search over hash_off.
+// Per request: first_miss = atomicMin over missing lanes, max_hit = atomicMax over hits that are not
+// already behind a miss of their own warp; a small per-request kernel then writes k_total / n_gpu and
+// blanks hits that lie behind the first miss (rare), and re-arms the scratch for the next call.
+#include <stdio.h>
+
+#include "cw_internal.cuh"
+
+namespace {
+
+__device__ __forceinline__ uint4 ld_slot(const cw_slot* s) { return *reinterpret_cast<const uint4*>(s); }
+__device__ __forceinline__ u64 slot_key(const uint4& v) { return ((u64)v.y << 32) | v.x; }
+
+// returns slot index of `key` (already remapped) or ~0 if absent
+__device__ __forceinline__ u64 table_find(const cw_slot* table, u64 mask, u64 key, u32* loc) {
+    u64 i = key & mask;
+    for (u64 n = 0; n <= mask; ++n) {
+        const uint4 v = ld_slot(table + i);
+        const u64 k = slot_key(v);
+        if (k == key) {
+            *loc = v.z;
+            return i;
+        }
+        if (k == CW_KEY_EMPTY) break;
+        i = (i + 1) & mask;
+    }
+    *loc = CW_MISS;
+    return ~0ull;
+}
+
+__global__ void lookup_kernel(const cw_slot* table, u64 mask, const u64* keys, u32 n, u32* loc) {
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    u32 l;
+    table_find(table, mask, cw_remap_key(keys[i]), &l);
+    loc[i] = l;
+}
+
+__global__ void erase_kernel(cw_slot* table, u64 mask, const u64* keys, u32 n) {
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    u32 l;
+    u64 s = table_find(table, mask, cw_remap_key(keys[i]), &l);
+    if (s != ~0ull) table[s].key = CW_KEY_TOMB;  // idx stays 0xFFFFFFFF, loc is dead
+}
+
+__global__ void retag_kernel(cw_slot* table, u64 mask, const u64* keys, const u32* new_loc, u32 n) {
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    u32 l;
+    u64 s = table_find(table, mask, cw_remap_key(keys[i]), &l);
+    if (s != ~0ull) table[s].loc = new_loc[i];
+}
+
+__global__ void insert_claim_kernel(cw_slot* table, u64 mask, const u64* keys, u32 n, u32* ins_slot, u32* status) {
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const u64 key = cw_remap_key(keys[i]);
+    const u64 home = key & mask;
+    u64 pos = home, steps = 0;
+    u64 found = ~0ull;
+    for (;;) {
+        // walk until the key, the end of the cluster (EMPTY) or a full cycle; remember the first reusable slot
+        u64 cand = ~0ull, cand_expect = 0;
+        while (steps <= mask) {
+            const u64 k = *reinterpret_cast<volatile unsigned long long*>(&table[pos].key);
+            if (k == key) {
+                found = pos;
+                break;
+            }
+            if (k == CW_KEY_TOMB && cand == ~0ull) {
+                cand = pos;
+                cand_expect = CW_KEY_TOMB;
+            }
+            if (k == CW_KEY_EMPTY) {
+                if (cand == ~0ull) {
+                    cand = pos;
+                    cand_expect = CW_KEY_EMPTY;
+                }
+                break;
+            }
+            pos = (pos + 1) & mask;
+            ++steps;
+        }
+        if (found != ~0ull || cand == ~0ull) break;  // present, or table full
+        const u64 old = atomicCAS(reinterpret_cast<unsigned long long*>(&table[cand].key),
+                                  (unsigned long long)cand_expect, (unsigned long long)key);
+        if (old == cand_expect) {
+            table[cand].loc = CW_LOC_PENDING;
+            found = cand;
+            break;
+        }
+        if (old == key) {
+            found = cand;
+            break;
+        }
+        // another key took the slot: every slot before it is occupied by other keys for the rest of the
+        // batch, so the walk resumes there
+        pos = cand;
+        steps = (cand - home) & mask;
+    }
+    if (found != ~0ull) {
+        atomicMin(&table[found].idx, i);
+        ins_slot[i] = (u32)found;
+    } else {
+        ins_slot[i] = 0xFFFFFFFFu;
+        atomicOr(status, CWS_CAPACITY);
+    }
+}
+
+__global__ void insert_resolve_kernel(cw_slot* table, const u32* loc, u32 n, const u32* ins_slot, u32* winner_loc) {
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const u32 s = ins_slot[i];
+    if (s == 0xFFFFFFFFu) {
+        if (winner_loc) winner_loc[i] = CW_MISS;
+        return;
+    }
+    const u32 w = table[s].idx;
+    u32 l = *reinterpret_cast<volatile u32*>(&table[s].loc);
+    if (l == CW_LOC_PENDING) {  // claimed in this batch: the lowest input index owns it
+        l = loc[w];
+        if (w == i) table[s].loc = l;
+    }
+    if (winner_loc) winner_loc[i] = l;
+}
+
+__global__ void insert_reset_kernel(cw_slot* table, u32 n, const u32* ins_slot) {
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const u32 s = ins_slot[i];
+    if (s != 0xFFFFFFFFu && table[s].idx == i) table[s].idx = 0xFFFFFFFFu;
+}
+
+// ---------------------------------------------------------------------------------------------- match
+__global__ void __launch_bounds__(256) match_probe_kernel(const cw_slot* __restrict__ table, u64 mask,
+                                                          const u64* __restrict__ hashes,
+                                                          const u64* __restrict__ hash_off, u32 R, u32* first_miss,
+                                                          u32* max_hit, u32* host_hits, u32* hit_loc) {
+    const u64 total = hash_off[R];
+    const u32 lane = threadIdx.x & 31;
+    const u64 nwarps = ((u64)gridDim.x * blockDim.x) >> 5;
+    for (u64 w = ((u64)blockIdx.x * blockDim.x + threadIdx.x) >> 5; w * 32 < total; w += nwarps) {
+        const u64 g0 = w * 32, g = g0 + lane;
+        // largest r with hash_off[r] <= g0 (r < R), 32-ary search, warp-uniform
+        u32 lo = 0, hi = R;
+        while (hi - lo > 1) {
+            u32 step = (hi - lo + 31) >> 5;
+            u32 p = lo + lane * step;
+            bool ok = p < hi && hash_off[p] <= g0;
+            u32 cnt = __popc(__ballot_sync(0xffffffffu, ok));
+            u32 nlo = lo + (cnt - 1) * step;
+            hi = min(hi, nlo + step);
+            lo = nlo;
+        }
+        const bool active = g < total;
+        u32 r = lo;
+        u32 loc = CW_MISS;
+        if (active) {
+            while (g >= hash_off[r + 1]) ++r;  // skips empty requests; rare past the first iteration
+            table_find(table, mask, cw_remap_key(hashes[g]), &loc);
+        }
+        const u32 j = active ? (u32)(g - hash_off[r]) : 0;
+        const bool uniform = __all_sync(0xffffffffu, !active || r == lo);
+        const u32 act_mask = __ballot_sync(0xffffffffu, active);
+        if (uniform) {
+            const u32 miss_mask = __ballot_sync(0xffffffffu, active && loc == CW_MISS);
+            const u32 first = miss_mask ? (u32)__ffs(miss_mask) - 1 : 32;
+            const bool behind = lane > first;
+            if (behind) loc = CW_MISS;
+            const u32 hit_mask = act_mask & (first >= 32 ? 0xffffffffu : ((1u << first) - 1));
+            const u32 host_mask = __ballot_sync(0xffffffffu, active && loc != CW_MISS && (loc & CW_HOST_BIT));
+            if (lane == 0 && act_mask) {
+                if (miss_mask) atomicMin(&first_miss[r], j + first);
+                if (hit_mask) atomicMax(&max_hit[r], j + (32 - __clz(hit_mask)));
+                if (host_mask) atomicAdd(&host_hits[r], __popc(host_mask));
+            }
+        } else if (active) {
+            if (loc == CW_MISS) {
+                atomicMin(&first_miss[r], j);
+            } else {
+                atomicMax(&max_hit[r], j + 1);
+                if (loc & CW_HOST_BIT) atomicAdd(&host_hits[r], 1u);
+            }
+        }
+        if (active && hit_loc) hit_loc[g] = loc;
+    }
+}
+
+// one warp per request
+__global__ void __launch_bounds__(256) match_finish_kernel(const u64* __restrict__ hash_off, u32 R, u32* first_miss,
+                                                           u32* max_hit, u32* host_hits, u32* k_total, u32* n_gpu,
+                                                           u32* hit_loc, const cw_slot* __restrict__ table, u64 mask,
+                                                           const u64* __restrict__ hashes) {
+    const u32 lane = threadIdx.x & 31;
+    const u32 r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (r >= R) return;
+    const u64 h0 = hash_off[r];
+    const u32 n_r = (u32)(hash_off[r + 1] - h0);
+    const u32 k = min(first_miss[r], n_r);
+    const u32 mh = max_hit[r];
+    const u32 hh = host_hits[r];
+    u32 host_in_run = 0;
+    if (hh) {  // count host-tier blocks inside the run (re-probe when the caller did not ask for hit_loc)
+        for (u32 j = lane; j < k; j += 32) {
+            u32 loc;
+            if (hit_loc) loc = hit_loc[h0 + j];
+            else table_find(table, mask, cw_remap_key(hashes[h0 + j]), &loc);
+            host_in_run += (loc != CW_MISS && (loc & CW_HOST_BIT)) ? 1 : 0;
+        }
+#pragma unroll
+        for (int m = 16; m; m >>= 1) host_in_run += __shfl_xor_sync(0xffffffffu, host_in_run, m);
+    }
+    if (hit_loc && mh > k)  // resident blocks behind the first miss are not part of the prefix
+        for (u32 j = k + lane; j < mh; j += 32) hit_loc[h0 + j] = CW_MISS;
+    if (lane == 0) {
+        k_total[r] = k;
+        n_gpu[r] = k - host_in_run;
+        first_miss[r] = 0xFFFFFFFFu;  // re-arm
+        max_hit[r] = 0;
+        host_hits[r] = 0;
+    }
+}
+
+__global__ void blocks_update_kernel(const u32* ids, u32 n, u32 size, const u32* session, const u32* depth,
+                                     const u32* last_access, const u32* ref_flags, u32* m_session, u32* m_depth,
+                                     u32* m_last, u32* m_ref, u32* status) {
+    u32 i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const u32 b = ids[i];
+    if (b >= size) {
+        atomicOr(status, CWS_INVAL);
+        return;
+    }
+    if (session) m_session[b] = session[i];
+    if (depth) m_depth[b] = depth[i];
+    if (last_access) m_last[b] = last_access[i];
+    if (ref_flags) m_ref[b] = ref_flags[i];
+}
+
+inline u32 cdiv(u64 a, u32 b) { return (u32)((a + b - 1) / b); }
+
+}  // namespace
+
+int32_t cwi_table_lookup(cw_ctx* ctx, const u64* d_keys, u32 n, u32* d_loc) {
+    if (!n) return CW_OK;
+    lookup_kernel<<<cdiv(n, 256), 256, 0, ctx->s_main>>>(ctx->table, ctx->n_slots - 1, d_keys, n, d_loc);
+    CW_LAUNCH_CHECK(ctx);
+    return CW_OK;
+}
+int32_t cwi_table_erase(cw_ctx* ctx, const u64* d_keys, u32 n) {
+    if (!n) return CW_OK;
+    erase_kernel<<<cdiv(n, 256), 256, 0, ctx->s_main>>>(ctx->table, ctx->n_slots - 1, d_keys, n);
+    CW_LAUNCH_CHECK(ctx);
+    return CW_OK;
+}
+int32_t cwi_table_retag(cw_ctx* ctx, const u64* d_keys, const u32* d_new_loc, u32 n) {
+    if (!n) return CW_OK;
+    retag_kernel<<<cdiv(n, 256), 256, 0, ctx->s_main>>>(ctx->table, ctx->n_slots - 1, d_keys, d_new_loc, n);
+    CW_LAUNCH_CHECK(ctx);
+    return CW_OK;
+}
+int32_t cwi_table_insert(cw_ctx* ctx, const u64* d_keys, const u32* d_loc, u32 n, u32* d_winner_loc) {
+    if (!n) return CW_OK;
+    if (n > ctx->ins_cap) {  // grow the per-batch scratch (outside of graph capture)
+        if (ctx->ins_slot) CW_CUDA(ctx, cudaFree(ctx->ins_slot));
+        ctx->ins_slot = nullptr;
+        ctx->ins_cap = 0;
+        CW_CUDA(ctx, cudaMalloc(&ctx->ins_slot, (size_t)n * sizeof(u32)));
+        ctx->ins_cap = n;
+    }
+    const u64 mask = ctx->n_slots - 1;
+    insert_claim_kernel<<<cdiv(n, 256), 256, 0, ctx->s_main>>>(ctx->table, mask, d_keys, n, ctx->ins_slot,
+                                                               ctx->d_status);
+    CW_LAUNCH_CHECK(ctx);
+    insert_resolve_kernel<<<cdiv(n, 256), 256, 0, ctx->s_main>>>(ctx->table, d_loc, n, ctx->ins_slot, d_winner_loc);
+    CW_LAUNCH_CHECK(ctx);
+    insert_reset_kernel<<<cdiv(n, 256), 256, 0, ctx->s_main>>>(ctx->table, n, ctx->ins_slot);
+    CW_LAUNCH_CHECK(ctx);
+    return CW_OK;
+}
+
+int32_t cwi_match_prefix(cw_ctx* ctx, const u64* d_hashes, const u64* d_hash_off, u32 R, u32* d_k_total,
+                         u32* d_n_gpu, u32* d_hit_loc) {
+    if (!R) return CW_OK;
+    const u64 mask = ctx->n_slots - 1;
+    // enough warps to cover max_hashed_blocks once, capped at a few waves; the kernel grid-strides
+    u64 warps = (ctx->cfg.max_hashed_blocks + 31) / 32;
+    u64 blocks = (warps + 7) / 8;
+    u64 cap = (u64)ctx->n_sm * 8 * 4;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    match_probe_kernel<<<(u32)blocks, 256, 0, ctx->s_main>>>(ctx->table, mask, d_hashes, d_hash_off, R,
+                                                             ctx->m_first_miss, ctx->m_max_hit, ctx->m_host_hits,
+                                                             d_hit_loc);
+    CW_LAUNCH_CHECK(ctx);
+    match_finish_kernel<<<cdiv((u64)R * 32, 256), 256, 0, ctx->s_main>>>(d_hash_off, R, ctx->m_first_miss,
+                                                                         ctx->m_max_hit, ctx->m_host_hits, d_k_total,
+                                                                         d_n_gpu, d_hit_loc, ctx->table, mask,
+                                                                         d_hashes);
+    CW_LAUNCH_CHECK(ctx);
+    return CW_OK;
+}
+
+int32_t cwi_blocks_update(cw_ctx* ctx, u32 tier, const u32* d_ids, u32 n, const u32* d_session, const u32* d_depth,
+                          const u32* d_last_access, const u32* d_ref_flags) {
+    if (!n) return CW_OK;
+    blocks_update_kernel<<<cdiv(n, 256), 256, 0, ctx->s_main>>>(
+        d_ids, n, ctx->tier_size[tier], d_session, d_depth, d_last_access, d_ref_flags, ctx->meta_session[tier],
+        ctx->meta_depth[tier], ctx->meta_last_access[tier], ctx->meta_ref_flags[tier], ctx->d_status);
+    CW_LAUNCH_CHECK(ctx);
+    return CW_OK;
+}

@@ -1,0 +1,122 @@
+"""GPU parity — stage 1 (cw_hash_blocks) against the oracle, bit-exact, through the C ABI."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from harness import gen
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    from gpu_util import small_ctx
+    c = small_ctx(max_hashed_blocks=1 << 21)
+    yield c
+    c.close()
+
+
+def _check(ctx, tokens, tok_off, **kw):
+    from gpu_util import gpu_hash
+    got, ho, st = gpu_hash(ctx, tokens, tok_off, **kw)
+    okw = {k: v for k, v in kw.items() if k in ("salt", "start_block", "start_state")}
+    if "hashes" in kw:
+        okw["hashes"] = np.array(kw["hashes"], np.uint64)
+    exp, eho = oracle.hash_blocks(tokens, tok_off, **okw)
+    assert st == 0
+    assert (ho == eho).all()
+    bad = np.nonzero(got != exp)[0]
+    assert bad.size == 0, f"{bad.size} mismatches, first at {bad[:5]}"
+    return got
+
+
+def test_known_answer_vectors(ctx):
+    kat = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "hash_kat.json")))
+    from gpu_util import gpu_hash
+    for c in kat["cases"]:
+        tok = np.array(c["tokens"], np.int32)
+        got, _, st = gpu_hash(ctx, tok, [0, tok.size], salt=[int(c["salt"], 16)])
+        assert st == 0 and [f"{int(x):016x}" for x in got] == c["hashes"], c["name"]
+
+
+def test_ragged_requests_all_alignments_and_tails(ctx):
+    g = gen.rng(11, 0)
+    # empty, sub-block, exact blocks, one unit (256 blocks) -1/0/+1, several units with ragged tail; the
+    # cumulative offsets visit all four 4-byte alignments
+    lens = [0, 5, 16, 17, 31, 32, 16 * 255 + 1, 16 * 256 + 2, 16 * 257 + 3, 16 * 1000 + 7, 1, 16 * 31 + 15,
+            16 * 32, 16 * 33 + 9, 0, 16 * 513 + 6, 3]
+    tok_off = np.concatenate([[0], np.cumsum(lens)]).astype(np.uint64)
+    assert {int(o) % 4 for o in tok_off[:-1]} == {0, 1, 2, 3}
+    tokens = g.integers(0, gen.VOCAB, size=int(tok_off[-1]), dtype=np.int32)
+    salt = g.integers(0, 1 << 63, size=len(lens), dtype=np.uint64)
+    _check(ctx, tokens, tok_off, salt=salt)
+    _check(ctx, tokens, tok_off)  # NULL salt
+
+
+def test_extreme_token_values_and_reserved_seeds(ctx):
+    tok = np.array([0x7FFFFFFF, -1, -2147483648, 0] * 64, np.int32)
+    _check(ctx, tok, [0, 100, tok.size], salt=[0, 0xFFFFFFFFFFFFFFFF])
+
+
+def test_long_request_crosses_more_than_32_units(ctx):
+    g = gen.rng(12, 0)
+    n_blocks = 256 * 41 + 77  # 42 units: the look-back needs two 32-wide batches
+    lens = [3, 16 * n_blocks + 5, 16 * 300]
+    tok_off = np.concatenate([[0], np.cumsum(lens)]).astype(np.uint64)
+    tokens = g.integers(0, gen.VOCAB, size=int(tok_off[-1]), dtype=np.int32)
+    _check(ctx, tokens, tok_off, salt=[7, 8, 9])
+
+
+def test_resume_from_start_block(ctx):
+    g = gen.rng(13, 0)
+    lens = [16 * 9 + 3, 16 * 600, 7, 16 * 1300 + 15, 16 * 256]
+    tok_off = np.concatenate([[0], np.cumsum(lens)]).astype(np.uint64)
+    tokens = g.integers(0, gen.VOCAB, size=int(tok_off[-1]), dtype=np.int32)
+    salt = np.arange(1, 6, dtype=np.uint64)
+    cold, ho = oracle.hash_blocks(tokens, tok_off, salt=salt)
+    for sb in ([0, 0, 0, 0, 0], [9, 600, 0, 1300, 256], [3, 255, 0, 257, 1], [1, 512, 0, 1299, 255]):
+        state = np.array([cold[int(ho[r]) + sb[r] - 1] if sb[r] else 0 for r in range(5)], np.uint64)
+        init = np.full(cold.size, 0x1111111111111111, np.uint64)
+        got = _check(ctx, tokens, tok_off, salt=salt, start_block=sb, start_state=state, hashes=init)
+        for r in range(5):
+            lo = int(ho[r])
+            assert (got[lo:lo + sb[r]] == 0x1111111111111111).all()
+            assert (got[lo + sb[r]:int(ho[r + 1])] == cold[lo + sb[r]:int(ho[r + 1])]).all()
+
+
+def test_scaled_stress_queue_and_repeatability(ctx):
+    snap = gen.stress_snapshot(seed=5, S=8, L=32768, RB=1024, req_per_session=16, len_median=4096, len_min=64,
+                               len_max=32768)
+    a = _check(ctx, snap.tokens, snap.tok_off)
+    b = _check(ctx, snap.tokens, snap.tok_off)  # the self-cleaning control block: second call identical
+    assert (a == b).all()
+
+
+def test_inconsistent_offsets_are_reported_not_crashing(ctx):
+    from gpu_util import dev, zeros
+    tok = dev(np.zeros(64, np.int32))
+    tok_off = dev(np.array([0, 64], np.uint64))
+    bad_hash_off = dev(np.array([0, 3], np.uint64))  # should be 4
+    out = zeros(8, np.uint64)
+    ctx.hash_blocks(tok, tok_off, bad_hash_off, 1, out)
+    assert ctx.sync(check=False) == -1
+    assert ctx.sync(check=False) == 0  # status is reported once
+
+
+def test_host_side_argument_checks(ctx):
+    import paper_2606_16824_b200 as cw
+    from gpu_util import dev, zeros
+    tok = dev(np.zeros(64, np.int32))
+    off = dev(np.array([0, 64], np.uint64))
+    ho = dev(np.array([0, 4], np.uint64))
+    out = zeros(8, np.uint64)
+    for args in [(None, off, ho, 1, out), (tok, None, ho, 1, out), (tok, off, ho, 1, None),
+                 (tok.data_ptr() + 4, off, ho, 1, out), (tok, off, ho, 1 << 30, out)]:
+        with pytest.raises(cw.CwError) as e:
+            ctx.hash_blocks(*args)
+        assert e.value.code == cw.CW_E_INVAL
+    ctx.hash_blocks(tok, off, ho, 0, out)  # R = 0 is a no-op
+    assert ctx.sync(check=False) == 0

@@ -78,6 +78,10 @@ int32_t cw_create(const cw_config* cfg, cw_ctx** out);
 int32_t cw_destroy(cw_ctx* ctx);
 /* Waits for stream_main and stream_copy, then returns (and clears) the latched device status. */
 int32_t cw_sync(cw_ctx* ctx);
+/* Orders stream_main after every PCIe copy issued so far on stream_copy (event wait on the device, no host
+ * sync): work queued on stream_main afterwards — e.g. the next step's kernels, or a timing event — sees the
+ * swap-out data on the host. */
+int32_t cw_join_copy(cw_ctx* ctx);
 /* Text of the last CW_E_CUDA failure ("" if none).  Valid until the next call on this ctx. */
 const char* cw_last_error(cw_ctx* ctx);
 /* Number of kernels this ctx has launched so far (bench.py's gpu_launches). */
@@ -115,7 +119,7 @@ int32_t cw_match_prefix(cw_ctx* ctx, const uint64_t* d_hashes, const uint64_t* d
  *   d_order uint32[R]: the permutation (input indices in dispatch order)
  *   d_num_admit, d_deficit: device scalars.  Walk d_order; admit while count < max_admit and
  *          need + a <= free_blocks + evictable; stop at the first misfit; deficit = max(0, need - free_blocks).
- * R must be <= min(max_requests, 8192) in this build. */
+ * R must be <= max_requests (the rank sort costs R^2 key comparisons: meant for queues of a few thousand). */
 int32_t cw_schedule(cw_ctx* ctx, uint32_t R, const uint32_t* d_need, const uint32_t* d_n_gpu,
                     const uint64_t* d_arrival_seq, const uint32_t* d_req_id, uint32_t policy,
                     uint32_t free_blocks, uint32_t evictable, uint32_t max_admit, uint32_t* d_order,

@@ -31,6 +31,7 @@ void free_all(cw_ctx* c) {
         if (c->ev_gather[t]) cudaEventDestroy(c->ev_gather[t]);
         if (c->ev_copy[t]) cudaEventDestroy(c->ev_copy[t]);
     }
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
     cudaFree(c->d_status);
     if (c->h_status) cudaFreeHost(c->h_status);
     cudaFree(c->hash_ctl);
@@ -39,6 +40,8 @@ void free_all(cw_ctx* c) {
     cudaFree(c->m_first_miss);
     cudaFree(c->m_max_hit);
     cudaFree(c->m_host_hits);
+    cudaFree(c->sched_a);
+    cudaFree(c->sched_ticket);
     cudaFree(c->tau_q);
     cudaFree(c->out_score);
     cudaFree(c->out_id);
@@ -116,6 +119,9 @@ int32_t cw_create(const cw_config* cfg, cw_ctx** out) {
     CW_CUDA(c, dalloc_zero(&c->m_first_miss, cfg->max_requests, s, 0xFF));
     CW_CUDA(c, dalloc_zero(&c->m_max_hit, cfg->max_requests, s));
     CW_CUDA(c, dalloc_zero(&c->m_host_hits, cfg->max_requests, s));
+    // stage 2b
+    CW_CUDA(c, dalloc_zero(&c->sched_a, cfg->max_requests, s));
+    CW_CUDA(c, dalloc_zero(&c->sched_ticket, 1, s));
     // stage 3
     c->ev_cap = cfg->num_blocks > cfg->host_slots ? cfg->num_blocks : cfg->host_slots;
     CW_CUDA(c, dalloc_zero(&c->tau_q, cfg->max_sessions ? cfg->max_sessions : 1, s));
@@ -139,6 +145,7 @@ int32_t cw_create(const cw_config* cfg, cw_ctx** out) {
         CW_CUDA(c, cudaEventCreateWithFlags(&c->ev_gather[t], cudaEventDisableTiming));
         CW_CUDA(c, cudaEventCreateWithFlags(&c->ev_copy[t], cudaEventDisableTiming));
     }
+    CW_CUDA(c, cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
     c->copy_grid = cwi_copy_grid(c->n_sm);
     CW_CUDA(c, cudaStreamSynchronize(s));
     CW_CUDA(c, cudaGetLastError());
@@ -164,6 +171,13 @@ int32_t cw_sync(cw_ctx* ctx) {
     const u32 st = *ctx->h_status;
     if (st & CWS_INVAL) return CW_E_INVAL;
     if (st & CWS_CAPACITY) return CW_E_CAPACITY;
+    return CW_OK;
+}
+
+int32_t cw_join_copy(cw_ctx* ctx) {
+    if (!ctx) return CW_E_STATE;
+    CW_CUDA(ctx, cudaEventRecord(ctx->ev_join, ctx->s_copy));
+    CW_CUDA(ctx, cudaStreamWaitEvent(ctx->s_main, ctx->ev_join, 0));
     return CW_OK;
 }
 
@@ -196,7 +210,7 @@ int32_t cw_schedule(cw_ctx* ctx, uint32_t R, const uint32_t* d_need, const uint3
                     uint32_t evictable, uint32_t max_admit, uint32_t* d_order, uint32_t* d_num_admit,
                     uint32_t* d_deficit) {
     if (!ctx) return CW_E_STATE;
-    if (policy > 2 || !d_num_admit || !d_deficit || R > ctx->cfg.max_requests || R > 8192) return CW_E_INVAL;
+    if (policy > 2 || !d_num_admit || !d_deficit || R > ctx->cfg.max_requests) return CW_E_INVAL;
     if (R && (!d_need || !d_n_gpu || !d_arrival_seq || !d_req_id || !d_order)) return CW_E_INVAL;
     return cwi_schedule(ctx, R, d_need, d_n_gpu, d_arrival_seq, d_req_id, policy, free_blocks, evictable, max_admit,
                         d_order, d_num_admit, d_deficit);

@@ -461,7 +461,10 @@ int32_t cwi_score_evict(cw_ctx* ctx, u32 tick_now, u32 S, u32 F, const uint8_t* 
     u32 tiles = (a.M + CWE_TILE - 1) / CWE_TILE;
     int grid = g_evict_grid;
     if ((u32)grid > tiles) grid = tiles ? (int)tiles : 1;
-    evict_kernel<<<grid, CWE_THREADS, CWE_SMEM_BYTES, ctx->s_main>>>(a);
+    // cooperative launch: the CTAs wait on one another at the grid barriers, so co-residency must be guaranteed
+    void* kargs[] = {&a};
+    CW_CUDA(ctx, cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(evict_kernel), dim3(grid), dim3(CWE_THREADS),
+                                             kargs, CWE_SMEM_BYTES, ctx->s_main));
     CW_LAUNCH_CHECK(ctx);
     return CW_OK;
 }

@@ -66,7 +66,10 @@ struct __align__(128) HashSmem {
     u64 carry[2];
 };
 
-__device__ __forceinline__ u64 slot_base(const u64* hash_off, u32 r) { return (hash_off[r] >> CWH_UNIT_LOG2) + r; }
+// unit slots are numbered relative to the call's first hash (hash_off may be a slice of a longer CSR array)
+__device__ __forceinline__ u64 slot_base(const u64* hash_off, u64 h_first, u32 r) {
+    return ((hash_off[r] - h_first) >> CWH_UNIT_LOG2) + r;
+}
 
 __device__ __forceinline__ u64 pow_u64(u64 base, u32 e) {
     u64 r = 1;
@@ -98,13 +101,15 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, 4) hash_kernel(const HashArgs a
     if (warp == CWH_WARPS) {
         // ------------------------------------------------------------------ producer warp
         const u32 R = a.R;
-        u64 total_blocks = R ? a.hash_off[R] : 0;
+        const u64 h_first = R ? a.hash_off[0] : 0;
+        u64 total_blocks = R ? a.hash_off[R] - h_first : 0;
         u64 total_slots = 0;
         if (R) {
-            if (total_blocks > a.max_hashed || (a.hash_off[R] >> CWH_UNIT_LOG2) + R > a.agg_slots) {
+            if (a.hash_off[R] < h_first || total_blocks > a.max_hashed ||
+                (total_blocks >> CWH_UNIT_LOG2) + R > a.agg_slots) {
                 if (lane == 0 && blockIdx.x == 0) atomicOr(a.status, CWS_INVAL);
             } else {
-                total_slots = (a.hash_off[R] >> CWH_UNIT_LOG2) + R;
+                total_slots = (total_blocks >> CWH_UNIT_LOG2) + R;
             }
         }
         const u64 policy = policy_evict_first();
@@ -125,7 +130,7 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, 4) hash_kernel(const HashArgs a
                 while (hi - lo > 1) {
                     u32 step = (hi - lo + 31) >> 5;
                     u32 p = lo + lane * step;
-                    bool ok = p < hi && slot_base(a.hash_off, p) <= tk;
+                    bool ok = p < hi && slot_base(a.hash_off, h_first, p) <= tk;
                     u32 cnt = __popc(__ballot_sync(0xffffffffu, ok));
                     u32 nlo = lo + (cnt - 1) * step;
                     hi = min(hi, nlo + step);
@@ -135,7 +140,7 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, 4) hash_kernel(const HashArgs a
                 const u64 h0 = a.hash_off[r], n_r = a.hash_off[r + 1] - h0;
                 const u64 t0 = a.tok_off[r], len = a.tok_off[r + 1] - t0;
                 const u64 sb = a.start_block ? a.start_block[r] : 0;
-                const u64 t = tk - ((h0 >> CWH_UNIT_LOG2) + r);
+                const u64 t = tk - slot_base(a.hash_off, h_first, r);
                 if (a.tok_off[r + 1] < t0 || n_r != (len >> 4) || sb > n_r) {
                     if (lane == 0 && t == 0) atomicOr(a.status, CWS_INVAL);
                     continue;

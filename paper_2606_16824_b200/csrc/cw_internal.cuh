@@ -120,6 +120,9 @@ struct cw_ctx {
     u32* m_first_miss;
     u32* m_max_hit;
     u32* m_host_hits;
+    // stage 2b
+    u32* sched_a;       // a of every request in dispatch order (max_requests)
+    u32* sched_ticket;  // "last CTA done" counter, self-cleaning
     // stage 3
     u32* tau_q;
     u64* cand_score[2];

@@ -152,11 +152,11 @@ __global__ void __launch_bounds__(256) match_probe_kernel(const cw_slot* __restr
                                                           const u64* __restrict__ hashes,
                                                           const u64* __restrict__ hash_off, u32 R, u32* first_miss,
                                                           u32* max_hit, u32* host_hits, u32* hit_loc) {
-    const u64 total = hash_off[R];
+    const u64 h_first = hash_off[0], total = hash_off[R];  // hash_off may be a slice of a longer CSR array
     const u32 lane = threadIdx.x & 31;
     const u64 nwarps = ((u64)gridDim.x * blockDim.x) >> 5;
-    for (u64 w = ((u64)blockIdx.x * blockDim.x + threadIdx.x) >> 5; w * 32 < total; w += nwarps) {
-        const u64 g0 = w * 32, g = g0 + lane;
+    for (u64 w = ((u64)blockIdx.x * blockDim.x + threadIdx.x) >> 5; h_first + w * 32 < total; w += nwarps) {
+        const u64 g0 = h_first + w * 32, g = g0 + lane;
         // largest r with hash_off[r] <= g0 (r < R), 32-ary search, warp-uniform
         u32 lo = 0, hi = R;
         while (hi - lo > 1) {

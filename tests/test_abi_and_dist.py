@@ -1,0 +1,119 @@
+"""CPU-only checks of the boundary and of the host logic around it (no compute calls: there is no GPU here).
+
+* libcachewise.so builds for sm_100a, loads, and exports every symbol include/cachewise.h declares;
+* the Python binding declares the same set; the cw_config struct layouts agree (field by field);
+* host-side argument checks that need no device answer before any CUDA call;
+* bench.py's multi-rank aggregation (replicas, max-over-ranks time) on gloo, world_size 2.
+"""
+import ctypes as C
+import os
+import re
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "cachewise.h")
+
+
+def _declared():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(cw_[a-z_0-9]+)\s*\(", src)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2606_16824_b200 import build
+    import paper_2606_16824_b200 as cw
+    build.build()
+    return cw.lib()
+
+
+def test_library_exports_every_declared_symbol(lib):
+    import paper_2606_16824_b200 as cw
+    names = _declared()
+    assert len(names) >= 19 and "cw_hash_blocks" in names and "cw_swap_in" in names
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in cachewise.h but not exported"
+    assert sorted(cw.EXPORTS) == names, "binding and header disagree"
+    out = subprocess.check_output(["nm", "-D", "--defined-only", cw.LIB_PATH], text=True)
+    exported = sorted(l.split()[-1] for l in out.splitlines() if " T " in l)
+    assert [e for e in exported if e.startswith("cw_")] == names
+    assert not [e for e in exported if not e.startswith("cw_") and not e.startswith("_")], "stray exports"
+
+
+def test_config_struct_layout_matches_the_header():
+    """Compile a tiny C program against the header and compare offsets with the ctypes mirror."""
+    import paper_2606_16824_b200 as cw
+    fields = [f for f, _ in cw.CwConfig._fields_]
+    prog = "#include <stdio.h>\n#include <stddef.h>\n#include \"cachewise.h\"\nint main(){"
+    for f in fields:
+        prog += f'printf("%zu\\n", offsetof(cw_config, {f}));'
+    prog += 'printf("%zu\\n", sizeof(cw_config));return 0;}'
+    exe = os.path.join("/tmp", f"cw_layout_{os.getpid()}")
+    subprocess.run(["gcc", "-x", "c", "-", "-I", os.path.join(ROOT, "include"), "-o", exe], input=prog, text=True,
+                   check=True)
+    got = [int(x) for x in subprocess.check_output([exe], text=True).split()]
+    os.unlink(exe)
+    want = [getattr(cw.CwConfig, f).offset for f in fields] + [C.sizeof(cw.CwConfig)]
+    assert got == want
+
+
+def test_null_ctx_and_bad_config_are_rejected_without_a_device(lib):
+    import paper_2606_16824_b200 as cw
+    assert lib.cw_sync(None) == cw.CW_E_STATE
+    assert lib.cw_destroy(None) == cw.CW_E_STATE
+    assert lib.cw_join_copy(None) == cw.CW_E_STATE
+    assert lib.cw_hash_blocks(None, None, None, None, None, None, None, 1, None) == cw.CW_E_STATE
+    assert lib.cw_swap_in(None, None, None, None, 1) == cw.CW_E_STATE
+    assert lib.cw_launch_count(None) == 0
+    h = C.c_void_p()
+    assert lib.cw_create(None, C.byref(h)) == cw.CW_E_INVAL
+    bad = cw.CwConfig(num_blocks=16, table_log2_slots=4, block_tokens=32, max_requests=1)   # block_tokens != 16
+    assert lib.cw_create(C.byref(bad), C.byref(h)) == cw.CW_E_INVAL and not h
+    bad = cw.CwConfig(num_blocks=1024, table_log2_slots=10, block_tokens=16, max_requests=1)  # load factor > 0.5
+    assert lib.cw_create(C.byref(bad), C.byref(h)) == cw.CW_E_INVAL and not h
+    bad = cw.CwConfig(num_blocks=16, table_log2_slots=6, block_tokens=16, max_requests=1, n_chunks=2, chunk_bytes=24,
+                      chunk_stride=24, block_stride=48, d_pool=4096)                       # chunk_bytes % 16 != 0
+    assert lib.cw_create(C.byref(bad), C.byref(h)) == cw.CW_E_INVAL and not h
+
+
+_WORKER = r"""
+import os, sys
+sys.path.insert(0, {root!r})
+from harness import dist as hdist
+rank, local, world = hdist.init("gloo")
+assert world == 2
+hdist.barrier()
+# rank r processed (r+1)*1000 units in (r+1)*10 ms: whole job = 3000 units / 20 ms
+u, t = hdist.aggregate((rank + 1) * 1000, (rank + 1) * 10.0)
+assert (u, t) == (3000.0, 20.0), (u, t)
+v = hdist.throughput((rank + 1) * 1000, (rank + 1) * 10.0)
+assert abs(v - 150000.0) < 1e-6, v
+hdist.finalize()
+print("ok", rank)
+"""
+
+
+def test_replica_aggregation_world_size_2_gloo(tmp_path):
+    script = tmp_path / "w.py"
+    script.write_text(_WORKER.format(root=ROOT))
+    port = 29600 + os.getpid() % 300
+    procs = []
+    for r in range(2):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.STDOUT, text=True))
+    for p in procs:
+        out, _ = p.communicate(timeout=120)
+        assert p.returncode == 0 and "ok" in out, out
+
+
+def test_reference_arm_other_ranks_exit_without_work():
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"],
+                         env=env, capture_output=True, text=True, timeout=120)
+    assert out.returncode == 0 and out.stdout.strip() == ""

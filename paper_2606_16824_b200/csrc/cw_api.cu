@@ -34,9 +34,9 @@ void free_all(cw_ctx* c) {
     if (c->ev_join) cudaEventDestroy(c->ev_join);
     cudaFree(c->d_status);
     if (c->h_status) cudaFreeHost(c->h_status);
-    cudaFree(c->hash_ctl);
-    cudaFree(c->hash_agg);
-    cudaFree(c->hash_flag);
+    cudaFree(c->hash_unit_off);
+    cudaFree(c->hash_plan);
+    cudaFree(c->hash_rec);
     cudaFree(c->m_first_miss);
     cudaFree(c->m_max_hit);
     cudaFree(c->m_host_hits);
@@ -110,11 +110,10 @@ int32_t cw_create(const cw_config* cfg, cw_ctx** out) {
     CW_CUDA(c, cudaHostAlloc(reinterpret_cast<void**>(&c->h_status), sizeof(u32), cudaHostAllocDefault));
     *c->h_status = 0;
     // stage 1
-    c->hash_slots = (cfg->max_hashed_blocks >> CWH_UNIT_LOG2) + cfg->max_requests + 1;
-    CW_CUDA(c, dalloc_zero(&c->hash_ctl, 1, s));
-    CW_CUDA(c, dalloc_zero(&c->hash_agg, c->hash_slots, s));
-    CW_CUDA(c, dalloc_zero(&c->hash_flag, c->hash_slots, s));
     c->hash_grid = cwi_hash_grid(c->n_sm);
+    CW_CUDA(c, dalloc_zero(&c->hash_unit_off, (size_t)cfg->max_requests + 1, s));
+    CW_CUDA(c, dalloc_zero(&c->hash_plan, 2, s));
+    CW_CUDA(c, dalloc_zero(&c->hash_rec, (size_t)c->hash_grid, s));
     // stage 2a
     CW_CUDA(c, dalloc_zero(&c->m_first_miss, cfg->max_requests, s, 0xFF));
     CW_CUDA(c, dalloc_zero(&c->m_max_hit, cfg->max_requests, s));

@@ -4,19 +4,24 @@
 //   chain   H_j = A*H_{j-1} + c_j  (mod 2^64),  H_{-1} = fin(salt ^ K7)  or  start_state
 //
 // The chain is an affine recurrence whose multiplier is always a power of A, so it is a SCAN:
-//   warp   : inclusive scan over 32 blocks, step d uses the constant A^d
-//   CTA    : 8 warp aggregates combined by Horner with A^32
-//   request: units of 256 blocks; unit t's carry-in = A^(256 t)*seed + sum_{v<t} A^(256 (t-1-v)) * agg_v,
-//            where agg_v is unit v's carry-free aggregate — published to global memory as soon as it is
-//            known, so no unit ever waits on another unit's look-back (no serial chain across units).
+//   warp : inclusive scan over 32 blocks, step d uses the constant A^d
+//   CTA  : 8 warp aggregates combined by Horner with A^32; the running state is carried from one 256-block
+//          unit to the next in registers
+//   grid : the list of units (request-aligned runs of <= 256 blocks) is cut into gridDim.x CONTIGUOUS ranges
+//          of equal length, one per CTA.  A CTA therefore walks its requests sequentially and never waits on
+//          another CTA (no look-back, no spinning).  Only the first request of a range can have begun in an
+//          earlier range: that boundary segment is scanned with carry-in 0 and patched afterwards,
+//          H_j += A^(j-j0+1) * carry_in, by hash_fixup_kernel (linear in the carry, mod 2^64).
 //
-// Data movement: one producer warp per CTA takes unit tickets (atomic counter => forward progress without
-// any co-residency assumption), locates the request with a warp-wide 32-ary search over hash_off, and
-// issues ONE TMA bulk copy (cp.async.bulk, L2 evict-first) of the unit's 16 KiB of token ids into a
-// 3-stage shared-memory ring.  Requests start at arbitrary 4-byte alignment: the copy starts at the
-// 16-byte boundary below and the consumers funnel the `mis` leading words away in registers.
-// Consumers read shared memory conflict-free (lane = 16-byte quarter of a block, 512 contiguous bytes per
-// LDS.128), form quarter sums, and transpose-reduce them with 6 shuffles so that each lane owns one block.
+// Three launches per call:
+//   hash_plan_kernel   units per request -> exclusive scan unit_off[R+1]; validates the offsets
+//   hash_kernel        the streaming pass: one producer warp issues ONE TMA bulk copy (cp.async.bulk, L2
+//                      evict-first) of each unit's 16 KiB of token ids into a 3-stage shared-memory ring
+//                      (mbarrier full/empty); 8 consumer warps read conflict-free 16-byte quarters, 2 multiplies
+//                      per lane, 6-shuffle transposed reduction, fin, 5-step warp scan
+//   hash_fixup_kernel  boundary segments (about half a request per CTA: ~1% extra traffic)
+// Requests start at arbitrary 4-byte alignment: the copy starts at the 16-byte boundary below and the
+// consumers funnel the `mis` leading words away in registers.
 #include <stdio.h>
 
 #include "cw_internal.cuh"
@@ -36,24 +41,24 @@ struct HashArgs {
     const u64* salt;
     const u64* hash_off;
     u64* hashes;
-    cw_hash_ctl* ctl;
-    u64* agg;
-    u32* flag;
+    u64* unit_off;      // [R+1] exclusive scan of units per request
+    u64* plan;          // [0] total units
+    cw_hash_rec* rec;   // per CTA of hash_kernel
     u32* status;
-    u64 agg_slots;
     u64 max_hashed;
     u32 R;
 };
 
+enum { MODE_CONTINUE = 0, MODE_SEED = 1, MODE_ZERO = 2 };
+
 struct UnitInfo {
     u64 out_base;  // index in hashes[] of the unit's first block
-    u64 slot;      // aggregate slot of this unit
-    u64 seed;      // H_{-1} or start_state of the request
+    u64 seed;      // H_{-1} or start_state of the request (MODE_SEED)
     u32 valid;
-    u32 t;         // unit index inside the request
     u32 nblk;      // blocks in this unit (<= CWH_UNIT)
     u32 mis;       // leading words to skip in the staged copy (0..3)
-    u32 publish;   // 1 if a later unit of the same request exists
+    u32 mode;      // where the unit's carry-in comes from
+    u32 last;      // last unit of this CTA's range: record the chain state after it
     u32 pad[3];
 };
 
@@ -63,15 +68,9 @@ struct __align__(128) HashSmem {
     u64 full[CWH_STAGES];
     u64 empty[CWH_STAGES];
     u64 wagg[2][CWH_WARPS];
-    u64 carry[2];
 };
 
-// unit slots are numbered relative to the call's first hash (hash_off may be a slice of a longer CSR array)
-__device__ __forceinline__ u64 slot_base(const u64* hash_off, u64 h_first, u32 r) {
-    return ((hash_off[r] - h_first) >> CWH_UNIT_LOG2) + r;
-}
-
-__device__ __forceinline__ u64 pow_u64(u64 base, u32 e) {
+__device__ __forceinline__ u64 pow_u64(u64 base, u64 e) {
     u64 r = 1;
     while (e) {
         if (e & 1) r *= base;
@@ -83,11 +82,74 @@ __device__ __forceinline__ u64 pow_u64(u64 base, u32 e) {
 
 __device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" ::"n"(CWH_UNIT) : "memory"); }
 
+// ------------------------------------------------------------------------------------------------ plan
+__global__ void __launch_bounds__(1024) hash_plan_kernel(const HashArgs a) {
+    __shared__ u64 s_warp[32];
+    __shared__ u64 s_total;
+    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const u32 R = a.R;
+    bool too_big = false;
+    if (a.hash_off[R] < a.hash_off[0] || a.hash_off[R] - a.hash_off[0] > a.max_hashed) too_big = true;
+    u64 running = 0;
+    for (u32 base = 0; base < R; base += 1024) {
+        const u32 r = base + tid;
+        u64 T = 0;
+        if (r < R && !too_big) {
+            const u64 t0 = a.tok_off[r], t1 = a.tok_off[r + 1], h0 = a.hash_off[r], h1 = a.hash_off[r + 1];
+            const u64 sb = a.start_block ? a.start_block[r] : 0;
+            if (t1 < t0 || h1 < h0 || (h1 - h0) != ((t1 - t0) >> 4) || sb > h1 - h0) atomicOr(a.status, CWS_INVAL);
+            else T = (h1 - h0 - sb + CWH_UNIT - 1) >> CWH_UNIT_LOG2;
+        }
+        u64 inc = T;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            u64 y = shfl64_up(inc, d);
+            if (lane >= d) inc += y;
+        }
+        if (lane == 31) s_warp[warp] = inc;
+        __syncthreads();
+        if (warp == 0) {
+            u64 w = s_warp[lane], wi = w;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                u64 y = shfl64_up(wi, d);
+                if (lane >= d) wi += y;
+            }
+            s_warp[lane] = wi - w;
+            if (lane == 31) s_total = wi;
+        }
+        __syncthreads();
+        if (r < R) a.unit_off[r] = running + s_warp[warp] + inc - T;
+        running += s_total;
+        __syncthreads();
+    }
+    if (tid == 0) {
+        a.unit_off[R] = running;
+        a.plan[0] = running;
+        if (too_big) atomicOr(a.status, CWS_INVAL);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ main pass
 __global__ void __launch_bounds__(CWH_UNIT + 32, 4) hash_kernel(const HashArgs a) {
     extern __shared__ __align__(128) uint8_t smem_raw[];
     HashSmem& sm = *reinterpret_cast<HashSmem*>(smem_raw);
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const u32 cur_epoch = a.ctl->epoch + 1;
+
+    const u64 U = a.plan[0];
+    const u64 per = (U + gridDim.x - 1) / gridDim.x;
+    const u64 u_begin = min(U, per * blockIdx.x), u_end = min(U, u_begin + per);
+    if (u_begin >= u_end) {  // empty range (uniform over the CTA): nothing to patch, nothing to hand on
+        if (tid == 0) {
+            cw_hash_rec rc;
+            rc.bseg_first = 0;
+            rc.tail_state = 0;
+            rc.bseg_len = 0;
+            rc.flags = 0;
+            a.rec[blockIdx.x] = rc;
+        }
+        return;
+    }
 
     if (tid == 0) {
         for (int s = 0; s < CWH_STAGES; ++s) {
@@ -101,78 +163,87 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, 4) hash_kernel(const HashArgs a
     if (warp == CWH_WARPS) {
         // ------------------------------------------------------------------ producer warp
         const u32 R = a.R;
-        const u64 h_first = R ? a.hash_off[0] : 0;
-        u64 total_blocks = R ? a.hash_off[R] - h_first : 0;
-        u64 total_slots = 0;
-        if (R) {
-            if (a.hash_off[R] < h_first || total_blocks > a.max_hashed ||
-                (total_blocks >> CWH_UNIT_LOG2) + R > a.agg_slots) {
-                if (lane == 0 && blockIdx.x == 0) atomicOr(a.status, CWS_INVAL);
-            } else {
-                total_slots = (total_blocks >> CWH_UNIT_LOG2) + R;
-            }
+        // largest r with unit_off[r] <= u_begin (=> unit_off[r+1] > u_begin), 32-ary search
+        u32 lo = 0, hi = R;
+        while (hi - lo > 1) {
+            u32 step = (hi - lo + 31) >> 5;
+            u32 p = lo + lane * step;
+            bool ok = p < hi && a.unit_off[p] <= u_begin;
+            u32 cnt = __popc(__ballot_sync(0xffffffffu, ok));
+            u32 nlo = lo + (cnt - 1) * step;
+            hi = min(hi, nlo + step);
+            lo = nlo;
         }
-        const u64 policy = policy_evict_first();
-        for (u32 it = 0;; ++it) {
-            const u32 s = it % CWH_STAGES;
-            if (it >= CWH_STAGES) mbar_wait(smem_u32(&sm.empty[s]), ((it / CWH_STAGES) - 1) & 1);
-            UnitInfo ui;
-            ui.valid = 0;
-            const i32* src = nullptr;
-            u32 bytes = 0;
-            for (;;) {
-                u64 tk = 0;
-                if (lane == 0) tk = atomicAdd(&a.ctl->ticket, 1u);
-                tk = shfl64(tk, 0);
-                if (tk >= total_slots) break;
-                // largest r with slot_base(r) <= tk, by 32-ary search (slot_base is strictly increasing)
-                u32 lo = 0, hi = R;
-                while (hi - lo > 1) {
-                    u32 step = (hi - lo + 31) >> 5;
-                    u32 p = lo + lane * step;
-                    bool ok = p < hi && slot_base(a.hash_off, h_first, p) <= tk;
-                    u32 cnt = __popc(__ballot_sync(0xffffffffu, ok));
-                    u32 nlo = lo + (cnt - 1) * step;
-                    hi = min(hi, nlo + step);
-                    lo = nlo;
+        if (lane == 0) {
+            const u64 policy = policy_evict_first();
+            u32 r = lo;
+            u64 u = u_begin;
+            u64 uo0 = a.unit_off[r], uo1 = a.unit_off[r + 1];
+            u64 t = u - uo0;
+            const bool starts_mid = t > 0;  // the first request began in an earlier CTA's range
+            bool in_bseg = starts_mid;
+            u64 bseg_first = 0, bseg_len = 0;
+            u64 h0 = 0, n_r = 0, t0 = 0, sb = 0, seed = 0;
+            bool fresh = true;
+            u32 it = 0;
+            for (; u < u_end; ++u, ++it) {
+                if (fresh) {
+                    h0 = a.hash_off[r];
+                    n_r = a.hash_off[r + 1] - h0;
+                    t0 = a.tok_off[r];
+                    sb = a.start_block ? a.start_block[r] : 0;
+                    seed = sb > 0 ? a.start_state[r] : cw_fin((a.salt ? a.salt[r] : 0ull) ^ CW_K7);
+                    fresh = false;
                 }
-                const u32 r = lo;
-                const u64 h0 = a.hash_off[r], n_r = a.hash_off[r + 1] - h0;
-                const u64 t0 = a.tok_off[r], len = a.tok_off[r + 1] - t0;
-                const u64 sb = a.start_block ? a.start_block[r] : 0;
-                const u64 t = tk - slot_base(a.hash_off, h_first, r);
-                if (a.tok_off[r + 1] < t0 || n_r != (len >> 4) || sb > n_r) {
-                    if (lane == 0 && t == 0) atomicOr(a.status, CWS_INVAL);
-                    continue;
-                }
-                const u64 todo = n_r - sb;
-                const u64 T = (todo + CWH_UNIT - 1) >> CWH_UNIT_LOG2;
-                if (t >= T) continue;  // unused slot of the sparse numbering
+                const u32 s = it % CWH_STAGES;
+                if (it >= CWH_STAGES) mbar_wait(smem_u32(&sm.empty[s]), ((it / CWH_STAGES) - 1) & 1);
                 const u64 j0 = sb + (t << CWH_UNIT_LOG2);
+                UnitInfo ui;
                 ui.valid = 1;
-                ui.t = (u32)t;
                 ui.nblk = (u32)min((u64)CWH_UNIT, n_r - j0);
                 ui.mis = (u32)(t0 & 3);
-                ui.publish = (t + 1 < T) ? 1u : 0u;
+                ui.mode = t == 0 ? MODE_SEED : (u == u_begin ? MODE_ZERO : MODE_CONTINUE);
                 ui.out_base = h0 + j0;
-                ui.slot = tk;
-                ui.seed = sb > 0 ? a.start_state[r] : cw_fin((a.salt ? a.salt[r] : 0ull) ^ CW_K7);
-                src = a.tokens + (t0 + 16 * j0 - ui.mis);
-                bytes = ui.nblk * 64 + (ui.mis ? 16u : 0u);
-                break;
-            }
-            if (lane == 0) {
+                ui.seed = seed;
+                ui.last = (u + 1 == u_end) ? 1u : 0u;
+                if (in_bseg) {
+                    if (u == u_begin) bseg_first = h0 + j0;
+                    bseg_len += ui.nblk;
+                }
                 sm.info[s] = ui;
+                const i32* src = a.tokens + (t0 + 16 * j0 - ui.mis);
+                const u32 bytes = ui.nblk * 64 + (ui.mis ? 16u : 0u);
                 const u32 bar = smem_u32(&sm.full[s]);
-                if (ui.valid) {
-                    mbar_expect_tx(bar, bytes);
-                    bulk_g2s(smem_u32(&sm.stage[s][0]), src, bytes, bar, policy);
-                } else {
-                    mbar_arrive(bar);
+                mbar_expect_tx(bar, bytes);
+                bulk_g2s(smem_u32(&sm.stage[s][0]), src, bytes, bar, policy);
+                // advance
+                ++t;
+                if (uo0 + t == uo1 && u + 1 < u_end) {
+                    in_bseg = false;
+                    do {
+                        ++r;
+                        uo0 = uo1;
+                        uo1 = a.unit_off[r + 1];
+                    } while (uo1 == uo0);  // requests without work
+                    t = 0;
+                    fresh = true;
                 }
             }
-            __syncwarp();
-            if (!ui.valid) break;
+            // terminator
+            {
+                const u32 s = it % CWH_STAGES;
+                if (it >= CWH_STAGES) mbar_wait(smem_u32(&sm.empty[s]), ((it / CWH_STAGES) - 1) & 1);
+                UnitInfo ui;
+                ui.valid = 0;
+                sm.info[s] = ui;
+                mbar_arrive(smem_u32(&sm.full[s]));
+            }
+            // hand-over record (tail_state is written by the consumers)
+            const bool tail_open = (uo0 + t) < uo1;  // the last request continues in the next range
+            a.rec[blockIdx.x].bseg_first = bseg_first;
+            a.rec[blockIdx.x].bseg_len = (u32)bseg_len;
+            a.rec[blockIdx.x].flags = (starts_mid ? CWH_REC_MID : 0u) | (in_bseg ? CWH_REC_TAIL_IS_BSEG : 0u) |
+                                      (tail_open ? CWH_REC_TAIL_OPEN : 0u);
         }
     } else {
         // ------------------------------------------------------------------ consumer warps
@@ -186,7 +257,8 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, 4) hash_kernel(const HashArgs a
         // the lane that owns block b is 4*(b&7) | ((b>>3)&1)<<1 | (b>>4)
         const u32 owner = ((lane & 7) << 2) | (((lane >> 3) & 1) << 1) | (lane >> 4);
         constexpr u64 A2 = cw_pow(CW_A, 2), A4 = cw_pow(CW_A, 4), A8 = cw_pow(CW_A, 8), A16 = cw_pow(CW_A, 16),
-                      A32 = cw_pow(CW_A, 32), AC = cw_pow(CW_A, CWH_UNIT);
+                      A32 = cw_pow(CW_A, 32);
+        u64 carry = 0;  // chain state before the current unit (uniform over the CTA)
 
         for (u32 it = 0;; ++it) {
             const u32 s = it % CWH_STAGES;
@@ -238,55 +310,49 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, 4) hash_kernel(const HashArgs a
             consumer_bar();
             if (tid == 0) mbar_arrive(smem_u32(&sm.empty[s]));  // every consumer has read stage s
 
-            if (warp == 0) {
-                if (ui.publish) {  // full unit: aggregate = sum_w A^(32 (W-1-w)) * wagg[w]
-                    u64 v = 0;
-                    if (lane < CWH_WARPS) v = sm.wagg[buf][lane] * pow_u64(A32, CWH_WARPS - 1 - lane);
+            // ---- carry-in of this warp by Horner over the earlier warps; the full Horner gives the next carry
+            u64 run = ui.mode == MODE_SEED ? ui.seed : (ui.mode == MODE_ZERO ? 0ull : carry);
+            u64 cin = 0;
 #pragma unroll
-                    for (int m = 1; m < CWH_WARPS; m <<= 1) v += shfl64_xor(v, m);
-                    if (lane == 0) {
-                        a.agg[ui.slot] = v;
-                        st_release_u32(&a.flag[ui.slot], cur_epoch);
-                    }
-                }
-                u64 carry = 0;
-                if (ui.t == 0) {
-                    carry = ui.seed;
-                } else {
-                    for (u32 b = 0; b < ui.t; b += 32) {
-                        const u32 v = b + lane;
-                        if (v < ui.t) {
-                            const u64 slot = ui.slot - ui.t + v;
-                            while (ld_acquire_u32(&a.flag[slot]) != cur_epoch) {
-                            }
-                            carry += ld_relaxed_u64(&a.agg[slot]) * pow_u64(AC, ui.t - 1 - v);
-                        }
-                    }
-                    if (lane == 0) carry += pow_u64(AC, ui.t) * ui.seed;
-#pragma unroll
-                    for (int m = 1; m < 32; m <<= 1) carry += shfl64_xor(carry, m);
-                }
-                if (lane == 0) sm.carry[buf] = carry;
+            for (u32 v = 0; v < CWH_WARPS; ++v) {
+                if (v == warp) cin = run;
+                run = A32 * run + sm.wagg[buf][v];
             }
-            consumer_bar();
-            u64 cin = sm.carry[buf];
-            for (u32 v = 0; v < warp; ++v) cin = A32 * cin + sm.wagg[buf][v];
+            carry = run;  // meaningful when the unit is full (a partial unit ends its request)
             const u64 h = x + a_lane1 * cin;
             const u32 bi = warp * 32 + lane;
             if (bi < ui.nblk) a.hashes[ui.out_base + bi] = h;
+            if (ui.last && tid == 0) a.rec[blockIdx.x].tail_state = carry;
         }
     }
+}
 
-    __syncthreads();
-    if (tid == 0) {
-        __threadfence();
-        const u32 prev = atomicAdd(&a.ctl->done, 1u);
-        if (prev == gridDim.x - 1) {  // last CTA: leave the control block ready for the next call
-            a.ctl->ticket = 0;
-            a.ctl->done = 0;
-            a.ctl->epoch = cur_epoch;
-            __threadfence();
+// ------------------------------------------------------------------------------------------------ fix-up
+// CTA c patches its boundary segment: H_j += A^(j-j0+1) * carry_in, where carry_in is the true chain state at
+// the end of range c-1 (itself patched through every earlier range that lies wholly inside the same request).
+__global__ void __launch_bounds__(256) hash_fixup_kernel(const HashArgs a, u32 n_ranges) {
+    const u32 c = blockIdx.x;
+    if (c == 0 || c >= n_ranges) return;
+    const cw_hash_rec me = a.rec[c];
+    if (!(me.flags & CWH_REC_MID) || me.bseg_len == 0) return;
+    __shared__ u64 s_carry;
+    if (threadIdx.x == 0) {
+        u64 acc = 0, mult = 1;
+        for (u32 k = c; k-- > 0;) {
+            const cw_hash_rec p = a.rec[k];
+            acc += mult * p.tail_state;
+            if (!(p.flags & CWH_REC_TAIL_IS_BSEG)) break;  // range k knew its own carry-in
+            mult *= pow_u64(CW_A, p.bseg_len);
         }
+        s_carry = acc;
+    }
+    __syncthreads();
+    const u64 carry = s_carry;
+    u64 m = pow_u64(CW_A, (u64)threadIdx.x + 1);
+    const u64 stride = pow_u64(CW_A, blockDim.x);
+    for (u32 j = threadIdx.x; j < me.bseg_len; j += blockDim.x) {
+        a.hashes[me.bseg_first + j] += m * carry;
+        m *= stride;
     }
 }
 
@@ -311,18 +377,23 @@ int32_t cwi_hash_blocks(cw_ctx* ctx, const i32* d_tokens, const u64* d_tok_off, 
     a.salt = d_salt;
     a.hash_off = d_hash_off;
     a.hashes = d_hashes;
-    a.ctl = ctx->hash_ctl;
-    a.agg = ctx->hash_agg;
-    a.flag = ctx->hash_flag;
+    a.unit_off = ctx->hash_unit_off;
+    a.plan = ctx->hash_plan;
+    a.rec = ctx->hash_rec;
     a.status = ctx->d_status;
-    a.agg_slots = ctx->hash_slots;
     a.max_hashed = ctx->cfg.max_hashed_blocks;
     a.R = R;
+    hash_plan_kernel<<<1, 1024, 0, ctx->s_main>>>(a);
+    CW_LAUNCH_CHECK(ctx);
     // never more CTAs than units could exist; small calls stay small
     u64 max_units = (ctx->cfg.max_hashed_blocks >> CWH_UNIT_LOG2) + R;
     int grid = (int)((u64)ctx->hash_grid < max_units ? (u64)ctx->hash_grid : max_units);
     if (grid < 1) grid = 1;
     hash_kernel<<<grid, CWH_UNIT + 32, sizeof(HashSmem), ctx->s_main>>>(a);
     CW_LAUNCH_CHECK(ctx);
+    if (grid > 1) {
+        hash_fixup_kernel<<<grid, 256, 0, ctx->s_main>>>(a, (u32)grid);
+        CW_LAUNCH_CHECK(ctx);
+    }
     return CW_OK;
 }

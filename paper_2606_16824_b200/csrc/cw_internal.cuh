@@ -64,12 +64,15 @@ __host__ __device__ __forceinline__ u64 cw_remap_key(u64 k) {
 #define CWH_STAGES 3                  // smem ring depth
 #define CWH_STAGE_BYTES (CWH_UNIT * 64 + 16)
 
-struct cw_hash_ctl {  // device-resident, self-cleaning (last CTA resets ticket/done and bumps epoch)
-    u32 ticket;
-    u32 done;
-    u32 epoch;
-    u32 pad;
+struct cw_hash_rec {  // what one CTA of hash_kernel hands to hash_fixup_kernel
+    u64 bseg_first;   // index in hashes[] of the first block of the boundary segment
+    u64 tail_state;   // chain state after the last block of the range (carry-free if TAIL_IS_BSEG)
+    u32 bseg_len;     // blocks of the range that belong to a request begun in an earlier range
+    u32 flags;
 };
+#define CWH_REC_MID 1u           // the range starts in the middle of a request
+#define CWH_REC_TAIL_IS_BSEG 2u  // the whole range lies inside that request
+#define CWH_REC_TAIL_OPEN 4u     // the last request of the range continues in the next range
 
 // ---- stage 3 scratch -------------------------------------------------------------------------------
 #define CWE_BINS 2048          // 11-bit digits
@@ -111,10 +114,9 @@ struct cw_ctx {
     u32* d_status;
     u32* h_status;  // pinned
     // stage 1
-    cw_hash_ctl* hash_ctl;
-    u64* hash_agg;
-    u32* hash_flag;
-    u64 hash_slots;
+    u64* hash_unit_off;  // max_requests + 1
+    u64* hash_plan;
+    cw_hash_rec* hash_rec;  // hash_grid
     int hash_grid;
     // stage 2a
     u32* m_first_miss;

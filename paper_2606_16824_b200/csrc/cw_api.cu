@@ -47,6 +47,7 @@ void free_all(cw_ctx* c) {
     cudaFree(c->out_id);
     cudaFree(c->hist);
     cudaFree(c->ev);
+    cudaFree(c->ev_rank);
     cudaFree(c->staging);
     if (c->own_copy_stream && c->s_copy) cudaStreamDestroy(c->s_copy);
 }
@@ -112,7 +113,7 @@ int32_t cw_create(const cw_config* cfg, cw_ctx** out) {
     // stage 1
     c->hash_grid = cwi_hash_grid(c->n_sm);
     CW_CUDA(c, dalloc_zero(&c->hash_unit_off, (size_t)cfg->max_requests + 1, s));
-    CW_CUDA(c, dalloc_zero(&c->hash_plan, 2, s));
+    CW_CUDA(c, dalloc_zero(&c->hash_plan, 4, s));
     CW_CUDA(c, dalloc_zero(&c->hash_rec, (size_t)c->hash_grid, s));
     // stage 2a
     CW_CUDA(c, dalloc_zero(&c->m_first_miss, cfg->max_requests, s, 0xFF));
@@ -132,6 +133,7 @@ int32_t cw_create(const cw_config* cfg, cw_ctx** out) {
     CW_CUDA(c, dalloc_zero(&c->out_id, c->ev_cap, s));
     CW_CUDA(c, dalloc_zero(&c->hist, (size_t)CWE_PASSES * CWE_BINS, s));
     CW_CUDA(c, dalloc_zero(&c->ev, 1, s));
+    CW_CUDA(c, dalloc_zero(&c->ev_rank, c->ev_cap, s));
     // stage 4
     if (cfg->staging_bytes) {
         if (!cfg->n_chunks || cfg->staging_bytes / 2 < c->page_bytes) {

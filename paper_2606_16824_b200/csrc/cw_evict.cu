@@ -1,15 +1,19 @@
 // Stage 3 — reuse-aware eviction (cw_score_evict).  DESIGN.md R4 / "Kernels: evict".
 //
-// ONE persistent kernel (grid = resident CTAs, hand-rolled grid barrier), phases:
+// ONE cooperative persistent kernel (one CTA per SM, hand-rolled grid barrier), phases:
 //   A  tau_q[s] per session: int32 dot product of uint8 features and int16 weights (PAPER.md 5.2 L217-219:
-//      one predicted time-to-next-reuse per session, L252), state overrides (L181, L277)
-//   B  per block: evictable? -> 64-bit fixed-point score -> compacted candidate list + histogram of the
-//      top 11 bits
-//   C  exact k-smallest of the 96-bit key (score : block id) by MSD radix select, 11 bits per pass: bins
-//      below the threshold bin are victims, the threshold bin becomes the next candidate list; stops as
-//      soon as the candidate list fits one CTA (<= 4096), which sorts it and takes what is still needed
-//   D  victims are sorted: 4096-element bitonic runs in shared memory, then a rank merge (each element's
-//      final position = its rank in its run + the number of smaller keys in every other run)
+//      one predicted time-to-next-reuse per session, L252), state overrides (L181, L277).  Every CTA
+//      computes all sessions into shared memory (S <= 4096), else one grid-wide pass through global memory.
+//   B  per block: evictable? -> 64-bit fixed-point score -> compacted candidate list + level-0 histogram
+//   C  exact k-smallest of the 96-bit key (score : block id) by MSD radix select, 11 bits per level.  The
+//      digit of a level is gathered from the top 11 bits that actually VARY inside the current candidate set
+//      (OR / AND masks accumulated while the set is written), so every level splits the set — no wasted
+//      levels when thousands of blocks share tau and age.  Bins below the threshold bin are victims, the
+//      threshold bin becomes the next candidate set; a set of <= 4096 is finished by one CTA in shared memory.
+//      Histograms use warp-aggregated shared-memory atomics (blocks of one session share a digit).
+//   D  victims are sorted by (score, id): 4096-element bitonic runs in shared memory, then a rank merge —
+//      for every (run, tile of victims) a CTA stages the run in shared memory and adds, for each victim of the
+//      tile, the number of smaller keys in that run to the victim's rank.
 //   E  scratch is re-zeroed for the next call (the kernel is self-cleaning => graph-capturable)
 // This replaces the paper's eviction heap + rebuild every N_rebuild=3 iterations (L252-254): a full
 // re-score and exact selection per call equals popping a heap rebuilt at this instant.
@@ -19,10 +23,13 @@
 
 namespace {
 
-#define CWE_THREADS 512
-#define CWE_ITEMS 4
+#define CWE_THREADS 1024
+#define CWE_WARPS (CWE_THREADS / 32)
+#define CWE_ITEMS 2
 #define CWE_TILE (CWE_THREADS * CWE_ITEMS)
-#define CWE_SMEM_BYTES (CWE_SORT_RUN * 12)
+#define CWE_SMEM_SESS 4096                       // sessions whose tau fits the per-CTA shared-memory table
+#define CWE_SMEM_SORT (CWE_SORT_RUN * 24)        // two (score,id) buffers of the CTA sort (alias the histogram)
+#define CWE_SMEM_BYTES (CWE_SMEM_SORT + CWE_SMEM_SESS * 4)
 
 struct EvictArgs {
     // inputs
@@ -43,8 +50,9 @@ struct EvictArgs {
     u32* cand_id[2];
     u64* out_score;
     u32* out_id;
+    u32* rank;       // aliases cand_id[0] (dead once the selection is over)
     u32* hist;       // [CWE_PASSES][CWE_BINS]
-    u32* counters;   // [0] n_out, [1] barrier count, [2] barrier generation, [4 + p] n_cand of pass p
+    cw_evict_state* st;
     u32* status;
     // outputs
     u32* victims;
@@ -52,63 +60,145 @@ struct EvictArgs {
     u32* num_victims;
 };
 
-__device__ __forceinline__ void grid_barrier(u32* count, u32* gen, u32 nblocks) {
+__device__ __forceinline__ void grid_barrier(cw_evict_state* st, u32 nblocks) {
     __syncthreads();
     if (threadIdx.x == 0) {
-        const u32 g = ld_acquire_u32(gen);
+        const u32 g = ld_acquire_u32(&st->bar_gen);
         __threadfence();
-        if (atomicAdd(count, 1u) == nblocks - 1) {
-            *count = 0;
+        if (atomicAdd(&st->bar_count, 1u) == nblocks - 1) {
+            st->bar_count = 0;
             __threadfence();
-            st_release_u32(gen, g + 1);
+            st_release_u32(&st->bar_gen, g + 1);
         } else {
-            while (ld_acquire_u32(gen) == g) {
+            while (ld_acquire_u32(&st->bar_gen) == g) {
             }
         }
         __threadfence();
     }
     __syncthreads();
-}
-
-__device__ __forceinline__ u32 key_digit(u64 score, u32 id, int p) {
-    int sh = 96 - CWE_DIGIT_BITS * (p + 1);
-    u32 width = CWE_DIGIT_BITS;
-    if (sh < 0) {
-        width = CWE_DIGIT_BITS + sh;
-        sh = 0;
-    }
-    u64 v;
-    if (sh >= 32) v = score >> (sh - 32);
-    else v = (score << (32 - sh)) | (u64)(id >> sh);
-    return (u32)v & ((1u << width) - 1);
 }
 
 __device__ __forceinline__ bool key_lt(u64 s1, u32 i1, u64 s2, u32 i2) { return s1 < s2 || (s1 == s2 && i1 < i2); }
 
-// bitonic sort of N (power of two) (score,id) keys in shared memory, ascending
-__device__ void smem_sort(u64* ss, u32* si, u32 N) {
-    for (u32 k = 2; k <= N; k <<= 1) {
-        for (u32 j = k >> 1; j > 0; j >>= 1) {
-            for (u32 t = threadIdx.x; t < (N >> 1); t += CWE_THREADS) {
-                const u32 i = ((t & ~(j - 1)) << 1) | (t & (j - 1));
-                const u32 p = i | j;
-                const bool up = (i & k) == 0;
-                const u64 xs = ss[i], ys = ss[p];
-                const u32 xi = si[i], yi = si[p];
-                if (key_lt(ys, yi, xs, xi) == up) {
-                    ss[i] = ys; si[i] = yi;
-                    ss[p] = xs; si[p] = xi;
-                }
-            }
-            __syncthreads();
+// ---- digit plan: up to 11 bit positions of the 96-bit key (95 = MSB of the score, 0 = LSB of the id), descending
+struct DigitPlan {
+    u32 nbits;
+    u32 pos[CWE_DIGIT_BITS];
+};
+__device__ __forceinline__ u32 key_bit(u64 score, u32 id, u32 pos) {
+    return pos >= 32 ? (u32)(score >> (pos - 32)) & 1u : (id >> pos) & 1u;
+}
+__device__ __forceinline__ u32 plan_digit(const DigitPlan& pl, u64 score, u32 id) {
+    u32 d = 0;
+#pragma unroll
+    for (int i = 0; i < CWE_DIGIT_BITS; ++i)
+        if (i < (int)pl.nbits) d = (d << 1) | key_bit(score, id, pl.pos[i]);
+    return d;
+}
+// the top 11 set bits of (vary_hi : vary_lo); then, if `fill_from` < 96, contiguous bits from there downwards
+__device__ __forceinline__ void make_plan(DigitPlan* pl, u64 vary_hi, u32 vary_lo, u32 fill_from) {
+    u32 n = 0;
+    u32 lowest = 96;
+    while (n < CWE_DIGIT_BITS && (vary_hi || vary_lo)) {
+        u32 p;
+        if (vary_hi) {
+            p = 63 - __clzll((long long)vary_hi);
+            vary_hi &= ~(1ull << p);
+            p += 32;
+        } else {
+            p = 31 - __clz((int)vary_lo);
+            vary_lo &= ~(1u << p);
         }
+        pl->pos[n++] = p;
+        lowest = p;
+    }
+    if (fill_from < 96) {
+        // plain bits below every chosen one keep the digit a monotone function of the key
+        u32 p = lowest == 96 ? fill_from : min(fill_from, lowest - 1);
+        while (n < CWE_DIGIT_BITS) {
+            pl->pos[n++] = p;
+            if (p == 0) break;
+            --p;
+        }
+    }
+    pl->nbits = n;
+}
+
+// CTA sort of N keys (score,id), N a power of two, 128 <= N <= CWE_SORT_RUN, ascending.
+//   1. every warp sorts 128-key chunks with a bitonic network in shared memory (__syncwarp only)
+//   2. log2(N/128) merge-path rounds between the two buffers: each thread finds its diagonal split by binary
+//      search and merges 4 consecutive outputs
+// On return (rs, ri) point at the buffer that holds the result.
+__device__ void cta_sort(u64* ss, u32* si, u64* ts, u32* ti, u32 N, u64*& rs, u32*& ri) {
+    const u32 lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (u32 chunk = warp; chunk < (N >> 7); chunk += CWE_WARPS) {
+        u64* cs = ss + (chunk << 7);
+        u32* ci = si + (chunk << 7);
+        for (u32 k = 2; k <= 128; k <<= 1) {
+            for (u32 j = k >> 1; j > 0; j >>= 1) {
+#pragma unroll
+                for (u32 q = 0; q < 2; ++q) {
+                    const u32 t = lane + 32 * q;
+                    const u32 i = ((t & ~(j - 1)) << 1) | (t & (j - 1));
+                    const u32 p = i | j;
+                    const bool up = (i & k) == 0;
+                    const u64 xs = cs[i], ys = cs[p];
+                    const u32 xi = ci[i], yi = ci[p];
+                    if (key_lt(ys, yi, xs, xi) == up) {
+                        cs[i] = ys; ci[i] = yi;
+                        cs[p] = xs; ci[p] = xi;
+                    }
+                }
+                __syncwarp();
+            }
+        }
+    }
+    for (u32 L = 128; L < N; L <<= 1) {
+        __syncthreads();
+        for (u32 o0 = threadIdx.x * 4; o0 < N; o0 += CWE_THREADS * 4) {
+            const u32 pair = o0 / (2 * L), d = o0 - pair * 2 * L;
+            const u64* As = ss + pair * 2 * L;
+            const u32* Ai = si + pair * 2 * L;
+            const u64* Bs = As + L;
+            const u32* Bi = Ai + L;
+            u32 lo = d > L ? d - L : 0, hi = min(d, L);
+            while (lo < hi) {  // how many of the first d outputs come from A
+                const u32 mid = (lo + hi) >> 1;
+                if (key_lt(As[mid], Ai[mid], Bs[d - 1 - mid], Bi[d - 1 - mid])) lo = mid + 1;
+                else hi = mid;
+            }
+            u32 x = lo, y = d - lo;
+#pragma unroll
+            for (u32 o = 0; o < 4; ++o) {
+                const bool take_a = y >= L || (x < L && key_lt(As[x], Ai[x], Bs[y], Bi[y]));
+                ts[o0 + o] = take_a ? As[x] : Bs[y];
+                ti[o0 + o] = take_a ? Ai[x] : Bi[y];
+                if (take_a) ++x;
+                else ++y;
+            }
+        }
+        u64* s_ = ss; ss = ts; ts = s_;
+        u32* i_ = si; si = ti; ti = i_;
+    }
+    __syncthreads();
+    rs = ss;
+    ri = si;
+}
+__device__ __forceinline__ u32 sort_size(u32 n) {  // power of two, at least one 128-key chunk
+    u32 N = 128;
+    while (N < n) N <<= 1;
+    return N;
+}
+// warp-aggregated shared-memory histogram increment (lanes of a warp mostly share a digit)
+__device__ __forceinline__ void hist_add(u32* s_hist, bool valid, u32 digit) {
+    const u32 act = __ballot_sync(0xffffffffu, valid);
+    if (valid) {
+        const u32 peers = __match_any_sync(act, digit);
+        if ((threadIdx.x & 31) == (u32)__ffs(peers) - 1) atomicAdd(&s_hist[digit], (u32)__popc(peers));
     }
 }
 
 // Block-cooperative compaction of one tile: flags f0 (-> list 0) and f1 (-> list 1) per item.
-struct TileOffsets {
-    u32 base0, base1;
-};
 __device__ __forceinline__ void tile_append(const bool (&f0)[CWE_ITEMS], const bool (&f1)[CWE_ITEMS],
                                             u32 (&pos0)[CWE_ITEMS], u32 (&pos1)[CWE_ITEMS], u32* ctr0, u32* ctr1,
                                             u32* s_w0, u32* s_w1, u32* s_base) {
@@ -130,7 +220,7 @@ __device__ __forceinline__ void tile_append(const bool (&f0)[CWE_ITEMS], const b
     }
     __syncthreads();
     if (warp == 0) {
-        u32 v0 = lane < CWE_THREADS / 32 ? s_w0[lane] : 0, v1 = lane < CWE_THREADS / 32 ? s_w1[lane] : 0;
+        u32 v0 = s_w0[lane], v1 = s_w1[lane];
         u32 i0 = v0, i1 = v1;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
@@ -140,10 +230,8 @@ __device__ __forceinline__ void tile_append(const bool (&f0)[CWE_ITEMS], const b
                 i1 += y1;
             }
         }
-        if (lane < CWE_THREADS / 32) {
-            s_w0[lane] = i0 - v0;
-            s_w1[lane] = i1 - v1;
-        }
+        s_w0[lane] = i0 - v0;
+        s_w1[lane] = i1 - v1;
         if (lane == 31) {
             s_base[0] = i0 ? atomicAdd(ctr0, i0) : 0;
             s_base[1] = i1 ? atomicAdd(ctr1, i1) : 0;
@@ -159,81 +247,191 @@ __device__ __forceinline__ void tile_append(const bool (&f0)[CWE_ITEMS], const b
     __syncthreads();  // s_w*/s_base are reused by the next tile
 }
 
-__global__ void __launch_bounds__(CWE_THREADS, 2) evict_kernel(const EvictArgs a) {
+// block-wide OR of a (u64,u32) pair of masks into global accumulators (one atomic per CTA and word)
+__device__ __forceinline__ void block_or_to_global(u64 hi, u32 lo, u64* g_hi, u32* g_lo, u64* s_hi, u32* s_lo) {
+    const u32 lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int m = 16; m; m >>= 1) {
+        hi |= shfl64_xor(hi, m);
+        lo |= __shfl_xor_sync(0xffffffffu, lo, m);
+    }
+    if (lane == 0) {
+        s_hi[warp] = hi;
+        s_lo[warp] = lo;
+    }
+    __syncthreads();
+    if (warp == 0) {
+        hi = s_hi[lane];
+        lo = s_lo[lane];
+#pragma unroll
+        for (int m = 16; m; m >>= 1) {
+            hi |= shfl64_xor(hi, m);
+            lo |= __shfl_xor_sync(0xffffffffu, lo, m);
+        }
+        if (lane == 0) {
+            if (hi) atomicOr(reinterpret_cast<unsigned long long*>(g_hi), (unsigned long long)hi);
+            if (lo) atomicOr(g_lo, lo);
+        }
+    }
+    __syncthreads();
+}
+
+// threshold bin of a level: the bin in which the `remaining`-th smallest candidate falls
+__device__ __forceinline__ void find_threshold(const u32* h, u32 remaining, u32* s_scan, u32* s_thr) {
+    constexpr int PER = CWE_BINS / CWE_THREADS;
+    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    u32 v[PER], sum = 0;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+        v[k] = __ldcg(h + tid * PER + k);
+        sum += v[k];
+    }
+    u32 inc = sum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        u32 y = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += y;
+    }
+    if (lane == 31) s_scan[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        u32 w = s_scan[lane], wi = w;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            u32 y = __shfl_up_sync(0xffffffffu, wi, d);
+            if (lane >= d) wi += y;
+        }
+        s_scan[lane] = wi - w;
+    }
+    __syncthreads();
+    u32 run = s_scan[warp] + inc - sum;  // exclusive prefix of this thread's first bin
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+        if (run < remaining && remaining <= run + v[k]) {
+            s_thr[0] = tid * PER + k;
+            s_thr[1] = run;
+            s_thr[2] = v[k];
+        }
+        run += v[k];
+    }
+    __syncthreads();
+}
+
+__device__ __forceinline__ void flush_hist(const u32* s_hist, u32* g_hist) {
+    __syncthreads();
+    for (u32 i = threadIdx.x; i < CWE_BINS; i += CWE_THREADS)
+        if (s_hist[i]) atomicAdd(&g_hist[i], s_hist[i]);
+}
+
+__global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     u32* s_hist = reinterpret_cast<u32*>(smem_raw);                       // phases B/C
     u64* s_score = reinterpret_cast<u64*>(smem_raw);                      // sorts
     u32* s_id = reinterpret_cast<u32*>(smem_raw + CWE_SORT_RUN * 8);
-    __shared__ u32 s_w0[CWE_THREADS / 32], s_w1[CWE_THREADS / 32], s_base[2];
-    __shared__ u32 s_scan[CWE_THREADS / 32];
+    u64* t_score = reinterpret_cast<u64*>(smem_raw + CWE_SORT_RUN * 12);
+    u32* t_id = reinterpret_cast<u32*>(smem_raw + CWE_SORT_RUN * 20);
+    u32* s_tau = reinterpret_cast<u32*>(smem_raw + CWE_SMEM_SORT);
+    __shared__ u32 s_w0[CWE_WARPS], s_w1[CWE_WARPS], s_base[2];
+    __shared__ u32 s_scan[CWE_WARPS];
     __shared__ u32 s_thr[3];  // threshold bin, count before it, count inside it
+    __shared__ u64 s_mhi[CWE_WARPS];
+    __shared__ u32 s_mlo[CWE_WARPS];
+    __shared__ u64 s_acc_hi;
+    __shared__ u32 s_acc_lo;
+    __shared__ DigitPlan s_plan;
     const u32 tid = threadIdx.x, G = gridDim.x;
-    u32* n_out = a.counters + 0;
-    u32* bar_count = a.counters + 1;
-    u32* bar_gen = a.counters + 2;
-    u32* n_cand = a.counters + 4;
+    cw_evict_state* st = a.st;
+    const bool tau_smem = a.S <= CWE_SMEM_SESS;
 
     // ---------------------------------------------------------------- A: per-session tau
-    for (u32 s = blockIdx.x * CWE_THREADS + tid; s < a.S; s += G * CWE_THREADS) {
-        const u32 st = a.session_state[s];
-        u32 tau;
-        if (st == CW_SESSION_QUEUED || st == CW_SESSION_RUNNING) {
-            tau = 0;
-        } else if (st >= CW_SESSION_IDLE) {
-            tau = CW_TAU_MAX;
-        } else if (a.tau_override) {
-            tau = min(a.tau_override[s], CW_TAU_MAX - 1);
-        } else {
-            i32 raw = a.bias;
-            for (u32 f = 0; f < a.F; ++f) raw += (i32)a.weights[f] * (i32)a.features[(u64)s * a.F + f];
-            tau = (u32)min(max(raw, 0), (i32)(CW_TAU_MAX - 1));
+    {
+        if (tid == 0) {
+            s_acc_hi = 0;
+            s_acc_lo = 0;
         }
-        a.tau_q[s] = tau;
+        __syncthreads();
+        u32 t_or = 0, t_nand = 0xFFFFFFu;  // over v = TAU_MAX - tau; v = 0 (idle / unknown session) always counts
+        const u32 s0 = tau_smem ? tid : blockIdx.x * CWE_THREADS + tid;
+        const u32 sstep = tau_smem ? CWE_THREADS : G * CWE_THREADS;
+        for (u32 s = s0; s < a.S; s += sstep) {
+            const u32 stt = a.session_state[s];
+            u32 tau;
+            if (stt == CW_SESSION_QUEUED || stt == CW_SESSION_RUNNING) {
+                tau = 0;
+            } else if (stt >= CW_SESSION_IDLE) {
+                tau = CW_TAU_MAX;
+            } else if (a.tau_override) {
+                tau = min(a.tau_override[s], CW_TAU_MAX - 1);
+            } else {
+                i32 raw = a.bias;
+                for (u32 f = 0; f < a.F; ++f) raw += (i32)a.weights[f] * (i32)a.features[(u64)s * a.F + f];
+                tau = (u32)min(max(raw, 0), (i32)(CW_TAU_MAX - 1));
+            }
+            if (tau_smem) s_tau[s] = tau;
+            else a.tau_q[s] = tau;
+            const u32 v = CW_TAU_MAX - tau;
+            t_or |= v;
+            t_nand |= ~v & 0xFFFFFFu;
+        }
+        const u64 packed = ((u64)t_or << 32) | t_nand;
+        if (tau_smem) {
+            block_or_to_global(packed, 0u, &s_acc_hi, &s_acc_lo, s_mhi, s_mlo);
+        } else {
+            block_or_to_global(packed, 0u, &st->tau_masks, &s_acc_lo, s_mhi, s_mlo);
+            grid_barrier(st, G);
+            if (tid == 0) s_acc_hi = __ldcg(reinterpret_cast<const unsigned long long*>(&st->tau_masks));
+            __syncthreads();
+        }
+        if (tid == 0) {
+            const u32 vary_tau = (u32)(s_acc_hi >> 32) & (u32)s_acc_hi & 0xFFFFFFu;
+            make_plan(&s_plan, (u64)vary_tau << 40, 0u, 39 + 32);
+        }
+        __syncthreads();
     }
-    grid_barrier(bar_count, bar_gen, G);
 
-    // ---------------------------------------------------------------- B: score + compact + histogram
+    // ---------------------------------------------------------------- B: score + compact + level-0 histogram
     for (u32 i = tid; i < CWE_BINS; i += CWE_THREADS) s_hist[i] = 0;
     __syncthreads();
-    for (u32 tile = blockIdx.x; (u64)tile * CWE_TILE < a.M; tile += G) {
-        bool f0[CWE_ITEMS], f1[CWE_ITEMS];
-        u32 p0[CWE_ITEMS], p1[CWE_ITEMS];
-        u64 sc[CWE_ITEMS];
+    {
+        const DigitPlan pl = s_plan;
+        for (u32 tile = blockIdx.x; (u64)tile * CWE_TILE < a.M; tile += G) {
+            bool f0[CWE_ITEMS], f1[CWE_ITEMS];
+            u32 p0[CWE_ITEMS], p1[CWE_ITEMS];
+            u64 sc[CWE_ITEMS];
 #pragma unroll
-        for (int k = 0; k < CWE_ITEMS; ++k) {
-            const u32 b = tile * CWE_TILE + k * CWE_THREADS + tid;
-            f0[k] = false;
-            f1[k] = false;
-            sc[k] = 0;
-            if (b < a.M) {
-                const u32 rf = a.m_ref[b];
-                if ((rf & CW_REF_VALID) && !(rf & CW_REF_PINNED) && (rf & 0x3FFFFFFFu) == 0) {
-                    const u32 sess = a.m_session[b];
-                    const u32 tau = sess < a.S ? a.tau_q[sess] : CW_TAU_MAX;
-                    const u32 la = a.m_last[b];
-                    const u32 age = min(a.tick_now >= la ? a.tick_now - la : 0u, 0xFFFFFu);
-                    const u32 dp = min(a.m_depth[b], 0xFFFFFu);
-                    sc[k] = ((u64)(CW_TAU_MAX - tau) << 40) | ((u64)(0xFFFFFu - age) << 20) | (u64)(0xFFFFFu - dp);
-                    f0[k] = true;
-                    atomicAdd(&s_hist[key_digit(sc[k], b, 0)], 1u);
+            for (int k = 0; k < CWE_ITEMS; ++k) {
+                const u32 b = tile * CWE_TILE + k * CWE_THREADS + tid;
+                f0[k] = false;
+                f1[k] = false;
+                sc[k] = 0;
+                if (b < a.M) {
+                    const u32 rf = a.m_ref[b];
+                    if ((rf & CW_REF_VALID) && !(rf & CW_REF_PINNED) && (rf & 0x3FFFFFFFu) == 0) {
+                        const u32 sess = a.m_session[b];
+                        const u32 tau = sess < a.S ? (tau_smem ? s_tau[sess] : __ldcg(a.tau_q + sess)) : CW_TAU_MAX;
+                        const u32 la = a.m_last[b];
+                        const u32 age = min(a.tick_now >= la ? a.tick_now - la : 0u, 0xFFFFFu);
+                        const u32 dp = min(a.m_depth[b], 0xFFFFFu);
+                        sc[k] = ((u64)(CW_TAU_MAX - tau) << 40) | ((u64)(0xFFFFFu - age) << 20) | (u64)(0xFFFFFu - dp);
+                        f0[k] = true;
+                    }
                 }
+                hist_add(s_hist, f0[k], f0[k] ? plan_digit(pl, sc[k], b) : 0u);
             }
-        }
-        tile_append(f0, f1, p0, p1, &n_cand[0], &n_cand[0], s_w0, s_w1, s_base);
+            tile_append(f0, f1, p0, p1, &st->n_cand[0], &st->n_cand[0], s_w0, s_w1, s_base);
 #pragma unroll
-        for (int k = 0; k < CWE_ITEMS; ++k)
-            if (f0[k]) {
-                a.cand_score[0][p0[k]] = sc[k];
-                a.cand_id[0][p0[k]] = tile * CWE_TILE + k * CWE_THREADS + tid;
-            }
+            for (int k = 0; k < CWE_ITEMS; ++k)
+                if (f0[k]) {
+                    a.cand_score[0][p0[k]] = sc[k];
+                    a.cand_id[0][p0[k]] = tile * CWE_TILE + k * CWE_THREADS + tid;
+                }
+        }
     }
-    __syncthreads();
-    for (u32 i = tid; i < CWE_BINS; i += CWE_THREADS)
-        if (s_hist[i]) atomicAdd(&a.hist[i], s_hist[i]);
-    grid_barrier(bar_count, bar_gen, G);
+    flush_hist(s_hist, a.hist);
+    grid_barrier(st, G);
 
     // ---------------------------------------------------------------- C: radix select
-    const u32 n_evictable = n_cand[0];
+    const u32 n_evictable = __ldcg(&st->n_cand[0]);
     const u32 asked = min(*a.deficit, a.cap);
     const u32 want = min(asked, n_evictable);
     if (blockIdx.x == 0 && tid == 0) {
@@ -249,69 +447,36 @@ __global__ void __launch_bounds__(CWE_THREADS, 2) evict_kernel(const EvictArgs a
             if (n_cur <= CWE_SMALL || p >= CWE_PASSES) {
                 // finish in one CTA: sort the candidates, take the first `remaining`
                 if (blockIdx.x == 0) {
-                    const u32 base = *n_out;
-                    for (u32 i = tid; i < CWE_SORT_RUN; i += CWE_THREADS) {
-                        s_score[i] = i < n_cur ? cs[i] : ~0ull;
-                        s_id[i] = i < n_cur ? ci[i] : 0xFFFFFFFFu;
+                    const u32 base = __ldcg(&st->n_out);
+                    const u32 N = sort_size(min(n_cur, (u32)CWE_SORT_RUN));
+                    __syncthreads();
+                    for (u32 i = tid; i < N; i += CWE_THREADS) {
+                        s_score[i] = i < n_cur ? __ldcg(cs + i) : ~0ull;
+                        s_id[i] = i < n_cur ? __ldcg(ci + i) : 0xFFFFFFFFu;
                     }
                     __syncthreads();
-                    smem_sort(s_score, s_id, CWE_SORT_RUN);
+                    u64* rs;
+                    u32* ri;
+                    cta_sort(s_score, s_id, t_score, t_id, N, rs, ri);
                     for (u32 i = tid; i < remaining; i += CWE_THREADS) {
-                        a.out_score[base + i] = s_score[i];
-                        a.out_id[base + i] = s_id[i];
+                        a.out_score[base + i] = rs[i];
+                        a.out_id[base + i] = ri[i];
                     }
                 }
                 break;
             }
-            // threshold bin of this pass (every CTA computes it redundantly from the global histogram)
-            {
-                const u32* h = a.hist + p * CWE_BINS;
-                constexpr int PER = CWE_BINS / CWE_THREADS;
-                u32 v[PER], sum = 0;
-#pragma unroll
-                for (int k = 0; k < PER; ++k) {
-                    v[k] = h[tid * PER + k];
-                    sum += v[k];
-                }
-                const u32 lane = tid & 31, warp = tid >> 5;
-                u32 inc = sum;
-#pragma unroll
-                for (int d = 1; d < 32; d <<= 1) {
-                    u32 y = __shfl_up_sync(0xffffffffu, inc, d);
-                    if (lane >= d) inc += y;
-                }
-                if (lane == 31) s_scan[warp] = inc;
-                __syncthreads();
-                if (warp == 0) {
-                    u32 w = lane < CWE_THREADS / 32 ? s_scan[lane] : 0, wi = w;
-#pragma unroll
-                    for (int d = 1; d < 32; d <<= 1) {
-                        u32 y = __shfl_up_sync(0xffffffffu, wi, d);
-                        if (lane >= d) wi += y;
-                    }
-                    if (lane < CWE_THREADS / 32) s_scan[lane] = wi - w;
-                }
-                __syncthreads();
-                u32 run = s_scan[warp] + inc - sum;  // exclusive prefix of this thread's first bin
-#pragma unroll
-                for (int k = 0; k < PER; ++k) {
-                    if (run < remaining && remaining <= run + v[k]) {
-                        s_thr[0] = tid * PER + k;
-                        s_thr[1] = run;
-                        s_thr[2] = v[k];
-                    }
-                    run += v[k];
-                }
-                __syncthreads();
-            }
+            // threshold bin of this level (every CTA computes it redundantly from the global histogram)
+            find_threshold(a.hist + p * CWE_BINS, remaining, s_scan, s_thr);
             const u32 thr = s_thr[0], before = s_thr[1], inside = s_thr[2];
             const u32 need_here = remaining - before;
             const bool take_all = need_here == inside;
-            // filter
-            for (u32 i = tid; i < CWE_BINS; i += CWE_THREADS) s_hist[i] = 0;
+            const DigitPlan pl = s_plan;
             __syncthreads();
+            // filter: bins below the threshold are victims, the threshold bin is the next candidate set
             u64* ns = a.cand_score[(p + 1) & 1];
             u32* ni = a.cand_id[(p + 1) & 1];
+            u64 m_or_hi = 0, m_nand_hi = 0;
+            u32 m_or_lo = 0, m_nand_lo = 0;
             for (u32 tile = blockIdx.x; (u64)tile * CWE_TILE < n_cur; tile += G) {
                 bool f0[CWE_ITEMS], f1[CWE_ITEMS];
                 u32 p0[CWE_ITEMS], p1[CWE_ITEMS];
@@ -324,17 +489,20 @@ __global__ void __launch_bounds__(CWE_THREADS, 2) evict_kernel(const EvictArgs a
                     sc[k] = 0;
                     id[k] = 0;
                     if (e < n_cur) {
-                        sc[k] = cs[e];
-                        id[k] = ci[e];
-                        const u32 dg = key_digit(sc[k], id[k], p);
+                        sc[k] = __ldcg(cs + e);
+                        id[k] = __ldcg(ci + e);
+                        const u32 dg = plan_digit(pl, sc[k], id[k]);
                         if (dg < thr || (take_all && dg == thr)) f0[k] = true;
                         else if (dg == thr) {
                             f1[k] = true;
-                            if (p + 1 < CWE_PASSES) atomicAdd(&s_hist[key_digit(sc[k], id[k], p + 1)], 1u);
+                            m_or_hi |= sc[k];
+                            m_nand_hi |= ~sc[k];
+                            m_or_lo |= id[k];
+                            m_nand_lo |= ~id[k];
                         }
                     }
                 }
-                tile_append(f0, f1, p0, p1, n_out, &n_cand[p + 1], s_w0, s_w1, s_base);
+                tile_append(f0, f1, p0, p1, &st->n_out, &st->n_cand[p + 1], s_w0, s_w1, s_base);
 #pragma unroll
                 for (int k = 0; k < CWE_ITEMS; ++k) {
                     if (f0[k]) {
@@ -346,70 +514,122 @@ __global__ void __launch_bounds__(CWE_THREADS, 2) evict_kernel(const EvictArgs a
                     }
                 }
             }
-            __syncthreads();
-            if (p + 1 < CWE_PASSES)
-                for (u32 i = tid; i < CWE_BINS; i += CWE_THREADS)
-                    if (s_hist[i]) atomicAdd(&a.hist[(p + 1) * CWE_BINS + i], s_hist[i]);
-            grid_barrier(bar_count, bar_gen, G);
+            if (!take_all && inside > CWE_SMALL) {
+                block_or_to_global(m_or_hi, m_or_lo, &st->or_hi[p + 1], &st->or_lo[p + 1], s_mhi, s_mlo);
+                block_or_to_global(m_nand_hi, m_nand_lo, &st->nand_hi[p + 1], &st->nand_lo[p + 1], s_mhi, s_mlo);
+            }
+            grid_barrier(st, G);
             if (take_all) {
                 remaining = 0;
                 break;
             }
             remaining = need_here;
             n_cur = inside;
+            if (n_cur <= CWE_SMALL || p + 1 >= CWE_PASSES) continue;  // finished by one CTA at the top of the loop
+            // histogram of the next level over the bits that still vary inside the new candidate set
+            if (tid == 0) {
+                const u64 vh = __ldcg(reinterpret_cast<const unsigned long long*>(&st->or_hi[p + 1])) &
+                               __ldcg(reinterpret_cast<const unsigned long long*>(&st->nand_hi[p + 1]));
+                const u32 vl = __ldcg(&st->or_lo[p + 1]) & __ldcg(&st->nand_lo[p + 1]);
+                make_plan(&s_plan, vh, vl, 96);
+            }
+            for (u32 i = tid; i < CWE_BINS; i += CWE_THREADS) s_hist[i] = 0;
+            __syncthreads();
+            {
+                const DigitPlan pn = s_plan;
+                for (u32 base = blockIdx.x * CWE_THREADS; base < n_cur; base += G * CWE_THREADS) {
+                    const u32 e = base + tid;
+                    const bool ok = e < n_cur;
+                    u32 dg = 0;
+                    if (ok) dg = plan_digit(pn, __ldcg(ns + e), __ldcg(ni + e));
+                    hist_add(s_hist, ok, dg);
+                }
+            }
+            flush_hist(s_hist, a.hist + (p + 1) * CWE_BINS);
+            grid_barrier(st, G);
         }
     }
-    grid_barrier(bar_count, bar_gen, G);
+    grid_barrier(st, G);
 
     // ---------------------------------------------------------------- E (early): re-zero scratch
-    // (nothing reads hist / n_cand / n_out any more: every CTA carries `want` in registers)
+    // (nothing reads hist / the state any more: every CTA carries `want` in registers)
     for (u32 i = blockIdx.x * CWE_THREADS + tid; i < CWE_PASSES * CWE_BINS; i += G * CWE_THREADS) a.hist[i] = 0;
-    if (blockIdx.x == 0 && tid < 4 + CWE_PASSES + 1 && tid != 1 && tid != 2) a.counters[tid] = 0;
+    if (blockIdx.x == 0) {
+        u32* w = reinterpret_cast<u32*>(st);
+        for (u32 i = 2 + tid; i < sizeof(cw_evict_state) / 4; i += CWE_THREADS) w[i] = 0;  // keeps bar_count/bar_gen
+    }
+    if (want == 0) return;
 
     // ---------------------------------------------------------------- D: sort the victims
     const u32 n_runs = (want + CWE_SORT_RUN - 1) / CWE_SORT_RUN;
     for (u32 run = blockIdx.x; run < n_runs; run += G) {
         const u32 lo = run * CWE_SORT_RUN, len = min((u32)CWE_SORT_RUN, want - lo);
-        for (u32 i = tid; i < CWE_SORT_RUN; i += CWE_THREADS) {
-            s_score[i] = i < len ? a.out_score[lo + i] : ~0ull;
-            s_id[i] = i < len ? a.out_id[lo + i] : 0xFFFFFFFFu;
+        const u32 N = sort_size(len);
+        __syncthreads();
+        for (u32 i = tid; i < N; i += CWE_THREADS) {
+            s_score[i] = i < len ? __ldcg(a.out_score + lo + i) : ~0ull;
+            s_id[i] = i < len ? __ldcg(a.out_id + lo + i) : 0xFFFFFFFFu;
         }
         __syncthreads();
-        smem_sort(s_score, s_id, CWE_SORT_RUN);
+        u64* rs;
+        u32* ri;
+        cta_sort(s_score, s_id, t_score, t_id, N, rs, ri);
         if (n_runs == 1) {
             for (u32 i = tid; i < len; i += CWE_THREADS) {
-                a.victims[i] = s_id[i];
-                if (a.victim_scores) a.victim_scores[i] = s_score[i];
+                a.victims[i] = ri[i];
+                if (a.victim_scores) a.victim_scores[i] = rs[i];
             }
         } else {
             for (u32 i = tid; i < len; i += CWE_THREADS) {
-                a.out_score[lo + i] = s_score[i];
-                a.out_id[lo + i] = s_id[i];
+                a.out_score[lo + i] = rs[i];
+                a.out_id[lo + i] = ri[i];
+                a.rank[lo + i] = i;  // rank inside its own run; the other runs are added below
             }
         }
-        __syncthreads();
     }
-    if (n_runs > 1) {
-        grid_barrier(bar_count, bar_gen, G);
-        for (u32 e = blockIdx.x * CWE_THREADS + tid; e < want; e += G * CWE_THREADS) {
-            const u64 s = a.out_score[e];
-            const u32 id = a.out_id[e];
-            const u32 my_run = e / CWE_SORT_RUN;
-            u32 rank = e - my_run * CWE_SORT_RUN;
-            for (u32 r = 0; r < n_runs; ++r) {
-                if (r == my_run) continue;
-                const u32 lo = r * CWE_SORT_RUN, len = min((u32)CWE_SORT_RUN, want - lo);
+    if (n_runs == 1) return;
+    grid_barrier(st, G);
+
+    // rank merge: item = (run r staged in shared memory, tile of victims searched in it)
+    {
+        const u64 work = (u64)want * n_runs;
+        u32 tile_e = (u32)((work + 2ull * G - 1) / (2ull * G));
+        tile_e = max(tile_e, (u32)CWE_THREADS);
+        const u32 tiles = (want + tile_e - 1) / tile_e;
+        const u32 items = n_runs * tiles;
+        u32 staged = 0xFFFFFFFFu;
+        for (u32 item = blockIdx.x; item < items; item += G) {
+            const u32 r = item / tiles, t = item - r * tiles;
+            const u32 lo = r * CWE_SORT_RUN, len = min((u32)CWE_SORT_RUN, want - lo);
+            if (staged != r) {
+                __syncthreads();
+                for (u32 i = tid; i < len; i += CWE_THREADS) {
+                    s_score[i] = __ldcg(a.out_score + lo + i);
+                    s_id[i] = __ldcg(a.out_id + lo + i);
+                }
+                __syncthreads();
+                staged = r;
+            }
+            const u32 e0 = t * tile_e, e1 = min(want, e0 + tile_e);
+            for (u32 e = e0 + tid; e < e1; e += CWE_THREADS) {
+                if (e >= lo && e < lo + len) continue;  // its own run
+                const u64 s = __ldcg(a.out_score + e);
+                const u32 id = __ldcg(a.out_id + e);
                 u32 l = 0, h = len;  // number of keys of run r below (s,id)
                 while (l < h) {
                     const u32 m = (l + h) >> 1;
-                    if (key_lt(a.out_score[lo + m], a.out_id[lo + m], s, id)) l = m + 1;
+                    if (key_lt(s_score[m], s_id[m], s, id)) l = m + 1;
                     else h = m;
                 }
-                rank += l;
+                if (l) atomicAdd(&a.rank[e], l);
             }
-            a.victims[rank] = id;
-            if (a.victim_scores) a.victim_scores[rank] = s;
         }
+    }
+    grid_barrier(st, G);
+    for (u32 e = blockIdx.x * CWE_THREADS + tid; e < want; e += G * CWE_THREADS) {
+        const u32 rk = __ldcg(a.rank + e);
+        a.victims[rk] = __ldcg(a.out_id + e);
+        if (a.victim_scores) a.victim_scores[rk] = __ldcg(a.out_score + e);
     }
 }
 
@@ -424,9 +644,11 @@ int32_t cwi_score_evict(cw_ctx* ctx, u32 tick_now, u32 S, u32 F, const uint8_t* 
         CW_CUDA(ctx, cudaFuncSetAttribute(evict_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CWE_SMEM_BYTES));
         int per_sm = 0;
         CW_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, evict_kernel, CWE_THREADS, CWE_SMEM_BYTES));
-        if (per_sm < 1) per_sm = 1;
-        if (per_sm > 2) per_sm = 2;
-        g_evict_grid = per_sm * ctx->n_sm;
+        if (per_sm < 1) {
+            snprintf(ctx->err, sizeof(ctx->err), "evict_kernel does not fit an SM");
+            return CW_E_CUDA;
+        }
+        g_evict_grid = ctx->n_sm;  // one CTA per SM: the cheapest grid barrier
     }
     EvictArgs a;
     a.features = d_features;
@@ -451,8 +673,9 @@ int32_t cwi_score_evict(cw_ctx* ctx, u32 tick_now, u32 S, u32 F, const uint8_t* 
     a.cand_id[1] = ctx->cand_id[1];
     a.out_score = ctx->out_score;
     a.out_id = ctx->out_id;
+    a.rank = ctx->ev_rank;
     a.hist = ctx->hist;
-    a.counters = reinterpret_cast<u32*>(ctx->ev);
+    a.st = ctx->ev;
     a.status = ctx->d_status;
     a.victims = d_victims;
     a.victim_scores = d_victim_scores;

@@ -10,16 +10,19 @@
 //   grid : the list of units (request-aligned runs of <= 256 blocks) is cut into gridDim.x CONTIGUOUS ranges
 //          of equal length, one per CTA.  A CTA therefore walks its requests sequentially and never waits on
 //          another CTA (no look-back, no spinning).  Only the first request of a range can have begun in an
-//          earlier range: that boundary segment is scanned with carry-in 0 and patched afterwards,
-//          H_j += A^(j-j0+1) * carry_in, by hash_fixup_kernel (linear in the carry, mod 2^64).
+//          earlier range: that boundary segment is scanned with carry-in 0 and patched at the very end of the
+//          CTA, H_j += A^(j-j0+1) * carry_in (linear in the carry, mod 2^64), once the CTA of the previous
+//          range has published its final chain state.  Ranges are handed out by an atomic ticket, so the
+//          CTA that is waited for has always started: the single wait per CTA cannot deadlock and happens
+//          when both CTAs are finishing anyway.
 //
-// Three launches per call:
+// Two launches per call:
 //   hash_plan_kernel   units per request -> exclusive scan unit_off[R+1]; validates the offsets
 //   hash_kernel        the streaming pass: one producer warp issues ONE TMA bulk copy (cp.async.bulk, L2
 //                      evict-first) of each unit's 16 KiB of token ids into a 3-stage shared-memory ring
 //                      (mbarrier full/empty); 8 consumer warps read conflict-free 16-byte quarters, 2 multiplies
-//                      per lane, 6-shuffle transposed reduction, fin, 5-step warp scan
-//   hash_fixup_kernel  boundary segments (about half a request per CTA: ~1% extra traffic)
+//                      per lane, 6-shuffle transposed reduction, fin, 5-step warp scan; then the boundary
+//                      patch (about half a request per CTA: ~1% extra traffic, L2-resident)
 // Requests start at arbitrary 4-byte alignment: the copy starts at the 16-byte boundary below and the
 // consumers funnel the `mis` leading words away in registers.
 #include <stdio.h>
@@ -42,7 +45,7 @@ struct HashArgs {
     const u64* hash_off;
     u64* hashes;
     u64* unit_off;      // [R+1] exclusive scan of units per request
-    u64* plan;          // [0] total units
+    u64* plan;          // [0] total units, [1] call epoch, [2] range ticket
     cw_hash_rec* rec;   // per CTA of hash_kernel
     u32* status;
     u64 max_hashed;
@@ -68,6 +71,12 @@ struct __align__(128) HashSmem {
     u64 full[CWH_STAGES];
     u64 empty[CWH_STAGES];
     u64 wagg[2][CWH_WARPS];
+    u64 carry_in;
+    u32 range;
+    u32 rec_flags;
+    u32 rec_bseg_len;
+    u64 rec_bseg_first;
+    u64 rec_tail_state;
 };
 
 __device__ __forceinline__ u64 pow_u64(u64 base, u64 e) {
@@ -83,50 +92,60 @@ __device__ __forceinline__ u64 pow_u64(u64 base, u64 e) {
 __device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" ::"n"(CWH_UNIT) : "memory"); }
 
 // ------------------------------------------------------------------------------------------------ plan
+__device__ __forceinline__ u64 plan_units(const HashArgs& a, u32 r, bool too_big) {
+    if (too_big) return 0;
+    const u64 t0 = a.tok_off[r], t1 = a.tok_off[r + 1], h0 = a.hash_off[r], h1 = a.hash_off[r + 1];
+    const u64 sb = a.start_block ? a.start_block[r] : 0;
+    if (t1 < t0 || h1 < h0 || (h1 - h0) != ((t1 - t0) >> 4) || sb > h1 - h0) return ~0ull;  // invalid request
+    return (h1 - h0 - sb + CWH_UNIT - 1) >> CWH_UNIT_LOG2;
+}
+
 __global__ void __launch_bounds__(1024) hash_plan_kernel(const HashArgs a) {
     __shared__ u64 s_warp[32];
-    __shared__ u64 s_total;
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const u32 R = a.R;
-    bool too_big = false;
-    if (a.hash_off[R] < a.hash_off[0] || a.hash_off[R] - a.hash_off[0] > a.max_hashed) too_big = true;
-    u64 running = 0;
-    for (u32 base = 0; base < R; base += 1024) {
-        const u32 r = base + tid;
-        u64 T = 0;
-        if (r < R && !too_big) {
-            const u64 t0 = a.tok_off[r], t1 = a.tok_off[r + 1], h0 = a.hash_off[r], h1 = a.hash_off[r + 1];
-            const u64 sb = a.start_block ? a.start_block[r] : 0;
-            if (t1 < t0 || h1 < h0 || (h1 - h0) != ((t1 - t0) >> 4) || sb > h1 - h0) atomicOr(a.status, CWS_INVAL);
-            else T = (h1 - h0 - sb + CWH_UNIT - 1) >> CWH_UNIT_LOG2;
-        }
-        u64 inc = T;
+    const bool too_big = a.hash_off[R] < a.hash_off[0] || a.hash_off[R] - a.hash_off[0] > a.max_hashed;
+    // every thread owns a contiguous run of requests: one round of loads, one block scan
+    const u32 per = (R + 1023) / 1024;
+    const u32 lo = min(R, tid * per), hi = min(R, lo + per);
+    u64 local = 0;
+    bool bad = false;
+    for (u32 r = lo; r < hi; ++r) {
+        const u64 T = plan_units(a, r, too_big);
+        if (T == ~0ull) bad = true;
+        else local += T;
+    }
+    if (bad) atomicOr(a.status, CWS_INVAL);
+    u64 inc = local;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        u64 y = shfl64_up(inc, d);
+        if (lane >= d) inc += y;
+    }
+    if (lane == 31) s_warp[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        u64 w = s_warp[lane], wi = w;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
-            u64 y = shfl64_up(inc, d);
-            if (lane >= d) inc += y;
+            u64 y = shfl64_up(wi, d);
+            if (lane >= d) wi += y;
         }
-        if (lane == 31) s_warp[warp] = inc;
-        __syncthreads();
-        if (warp == 0) {
-            u64 w = s_warp[lane], wi = w;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                u64 y = shfl64_up(wi, d);
-                if (lane >= d) wi += y;
-            }
-            s_warp[lane] = wi - w;
-            if (lane == 31) s_total = wi;
+        s_warp[lane] = wi - w;
+        if (lane == 31) {
+            a.unit_off[R] = wi;
+            a.plan[0] = wi;
+            a.plan[1] = a.plan[1] + 1;  // epoch of this call (ready flags of earlier calls become stale)
+            a.plan[2] = 0;              // range ticket
+            if (too_big) atomicOr(a.status, CWS_INVAL);
         }
-        __syncthreads();
-        if (r < R) a.unit_off[r] = running + s_warp[warp] + inc - T;
-        running += s_total;
-        __syncthreads();
     }
-    if (tid == 0) {
-        a.unit_off[R] = running;
-        a.plan[0] = running;
-        if (too_big) atomicOr(a.status, CWS_INVAL);
+    __syncthreads();
+    u64 run = s_warp[warp] + inc - local;
+    for (u32 r = lo; r < hi; ++r) {
+        a.unit_off[r] = run;
+        const u64 T = plan_units(a, r, too_big);
+        if (T != ~0ull) run += T;
     }
 }
 
@@ -136,20 +155,14 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, 4) hash_kernel(const HashArgs a
     HashSmem& sm = *reinterpret_cast<HashSmem*>(smem_raw);
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
+    if (tid == 0) sm.range = atomicAdd(reinterpret_cast<unsigned int*>(a.plan + 2), 1u);
+    __syncthreads();
+    const u32 range = sm.range;  // ranges in ticket order: every lower range belongs to a CTA that has started
     const u64 U = a.plan[0];
+    const u32 epoch = (u32)a.plan[1];
     const u64 per = (U + gridDim.x - 1) / gridDim.x;
-    const u64 u_begin = min(U, per * blockIdx.x), u_end = min(U, u_begin + per);
-    if (u_begin >= u_end) {  // empty range (uniform over the CTA): nothing to patch, nothing to hand on
-        if (tid == 0) {
-            cw_hash_rec rc;
-            rc.bseg_first = 0;
-            rc.tail_state = 0;
-            rc.bseg_len = 0;
-            rc.flags = 0;
-            a.rec[blockIdx.x] = rc;
-        }
-        return;
-    }
+    const u64 u_begin = min(U, per * range), u_end = min(U, u_begin + per);
+    if (u_begin >= u_end) return;  // empty range (uniform over the CTA): nobody waits for it
 
     if (tid == 0) {
         for (int s = 0; s < CWH_STAGES; ++s) {
@@ -238,12 +251,12 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, 4) hash_kernel(const HashArgs a
                 sm.info[s] = ui;
                 mbar_arrive(smem_u32(&sm.full[s]));
             }
-            // hand-over record (tail_state is written by the consumers)
+            // hand-over record (rec_tail_state is written by the consumers)
             const bool tail_open = (uo0 + t) < uo1;  // the last request continues in the next range
-            a.rec[blockIdx.x].bseg_first = bseg_first;
-            a.rec[blockIdx.x].bseg_len = (u32)bseg_len;
-            a.rec[blockIdx.x].flags = (starts_mid ? CWH_REC_MID : 0u) | (in_bseg ? CWH_REC_TAIL_IS_BSEG : 0u) |
-                                      (tail_open ? CWH_REC_TAIL_OPEN : 0u);
+            sm.rec_bseg_first = bseg_first;
+            sm.rec_bseg_len = (u32)bseg_len;
+            sm.rec_flags = (starts_mid ? CWH_REC_MID : 0u) | (in_bseg ? CWH_REC_TAIL_IS_BSEG : 0u) |
+                           (tail_open ? CWH_REC_TAIL_OPEN : 0u);
         }
     } else {
         // ------------------------------------------------------------------ consumer warps
@@ -322,37 +335,43 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, 4) hash_kernel(const HashArgs a
             const u64 h = x + a_lane1 * cin;
             const u32 bi = warp * 32 + lane;
             if (bi < ui.nblk) a.hashes[ui.out_base + bi] = h;
-            if (ui.last && tid == 0) a.rec[blockIdx.x].tail_state = carry;
+            if (ui.last && tid == 0) sm.rec_tail_state = carry;
         }
     }
-}
 
-// ------------------------------------------------------------------------------------------------ fix-up
-// CTA c patches its boundary segment: H_j += A^(j-j0+1) * carry_in, where carry_in is the true chain state at
-// the end of range c-1 (itself patched through every earlier range that lies wholly inside the same request).
-__global__ void __launch_bounds__(256) hash_fixup_kernel(const HashArgs a, u32 n_ranges) {
-    const u32 c = blockIdx.x;
-    if (c == 0 || c >= n_ranges) return;
-    const cw_hash_rec me = a.rec[c];
-    if (!(me.flags & CWH_REC_MID) || me.bseg_len == 0) return;
-    __shared__ u64 s_carry;
-    if (threadIdx.x == 0) {
-        u64 acc = 0, mult = 1;
-        for (u32 k = c; k-- > 0;) {
-            const cw_hash_rec p = a.rec[k];
-            acc += mult * p.tail_state;
-            if (!(p.flags & CWH_REC_TAIL_IS_BSEG)) break;  // range k knew its own carry-in
-            mult *= pow_u64(CW_A, p.bseg_len);
+    // ---- hand-over and boundary patch
+    __syncthreads();
+    const u32 flags = sm.rec_flags;
+    const u32 bseg_len = sm.rec_bseg_len;
+    if (tid == 0) {
+        const bool dependent = (flags & CWH_REC_TAIL_IS_BSEG) != 0;  // whole range inside one request
+        if (!dependent) {  // the tail is already final: publish before waiting, so waits never chain
+            a.rec[range].true_tail = sm.rec_tail_state;
+            st_release_u32(&a.rec[range].ready, epoch);
         }
-        s_carry = acc;
+        u64 carry_in = 0;
+        if (flags & CWH_REC_MID) {  // the true chain state at the end of the previous range
+            const cw_hash_rec* prev = a.rec + (range - 1);
+            while (ld_acquire_u32(&prev->ready) != epoch) {
+            }
+            carry_in = ld_relaxed_u64(&prev->true_tail);
+        }
+        if (dependent) {
+            a.rec[range].true_tail = sm.rec_tail_state + pow_u64(CW_A, bseg_len) * carry_in;
+            st_release_u32(&a.rec[range].ready, epoch);
+        }
+        sm.carry_in = carry_in;
     }
     __syncthreads();
-    const u64 carry = s_carry;
-    u64 m = pow_u64(CW_A, (u64)threadIdx.x + 1);
-    const u64 stride = pow_u64(CW_A, blockDim.x);
-    for (u32 j = threadIdx.x; j < me.bseg_len; j += blockDim.x) {
-        a.hashes[me.bseg_first + j] += m * carry;
-        m *= stride;
+    if ((flags & CWH_REC_MID) && bseg_len) {
+        const u64 carry_in = sm.carry_in;
+        const u64 first = sm.rec_bseg_first;
+        u64 m = pow_u64(CW_A, (u64)tid + 1);
+        const u64 stride = pow_u64(CW_A, blockDim.x);
+        for (u32 j = tid; j < bseg_len; j += blockDim.x) {
+            a.hashes[first + j] += m * carry_in;
+            m *= stride;
+        }
     }
 }
 
@@ -391,9 +410,5 @@ int32_t cwi_hash_blocks(cw_ctx* ctx, const i32* d_tokens, const u64* d_tok_off, 
     if (grid < 1) grid = 1;
     hash_kernel<<<grid, CWH_UNIT + 32, sizeof(HashSmem), ctx->s_main>>>(a);
     CW_LAUNCH_CHECK(ctx);
-    if (grid > 1) {
-        hash_fixup_kernel<<<grid, 256, 0, ctx->s_main>>>(a, (u32)grid);
-        CW_LAUNCH_CHECK(ctx);
-    }
     return CW_OK;
 }

@@ -64,11 +64,10 @@ __host__ __device__ __forceinline__ u64 cw_remap_key(u64 k) {
 #define CWH_STAGES 3                  // smem ring depth
 #define CWH_STAGE_BYTES (CWH_UNIT * 64 + 16)
 
-struct cw_hash_rec {  // what one CTA of hash_kernel hands to hash_fixup_kernel
-    u64 bseg_first;   // index in hashes[] of the first block of the boundary segment
-    u64 tail_state;   // chain state after the last block of the range (carry-free if TAIL_IS_BSEG)
-    u32 bseg_len;     // blocks of the range that belong to a request begun in an earlier range
-    u32 flags;
+struct cw_hash_rec {  // what the CTA of one range publishes for the CTA of the next range
+    u64 true_tail;  // chain state after the last block of the range
+    u32 ready;      // == call epoch once true_tail is final
+    u32 pad;
 };
 #define CWH_REC_MID 1u           // the range starts in the middle of a request
 #define CWH_REC_TAIL_IS_BSEG 2u  // the whole range lies inside that request
@@ -77,21 +76,19 @@ struct cw_hash_rec {  // what one CTA of hash_kernel hands to hash_fixup_kernel
 // ---- stage 3 scratch -------------------------------------------------------------------------------
 #define CWE_BINS 2048          // 11-bit digits
 #define CWE_DIGIT_BITS 11
-#define CWE_PASSES 9           // ceil(96/11): 64-bit score then 32-bit id
+#define CWE_PASSES 12          // level 0 (tau bits) + at most ceil(96/11) levels over bits that still vary
 #define CWE_SMALL 4096         // finish in one CTA when the candidate set is this small
 #define CWE_SORT_RUN 4096      // victims sorted in runs of this size, then rank-merged
 
-struct cw_evict_state {
-    u32 n_evictable;   // candidates appended by the score kernel
-    u32 want;          // min(deficit, cap, n_evictable)
-    u32 remaining;     // victims still to be taken from the current candidate set
-    u32 n_cand[2];     // candidate counts of the ping-pong buffers
-    u32 n_out;         // victims emitted so far (unsorted)
-    u32 done;          // selection finished
-    u32 pass;          // next digit index
-    u32 thr_digit;     // threshold digit of the current pass
-    u32 cur;           // which candidate buffer is current
-    u32 pad[6];
+struct cw_evict_state {  // all zero between calls, except the barrier words
+    u32 bar_count, bar_gen;           // grid barrier
+    u32 n_out;                        // victims emitted so far (unsorted)
+    u32 pad0;
+    u64 tau_masks;                    // OR of (TAU_MAX-tau) << 32 | OR of its complement (global-tau path)
+    u32 n_cand[CWE_PASSES + 1];       // candidates of every level
+    u32 pad1;
+    u32 or_lo[CWE_PASSES + 1], nand_lo[CWE_PASSES + 1];  // OR of the ids / of their complements, per level
+    u64 or_hi[CWE_PASSES + 1], nand_hi[CWE_PASSES + 1];  // same for the scores
 };
 
 struct cw_ctx {
@@ -133,6 +130,7 @@ struct cw_ctx {
     u32* out_id;
     u32* hist;  // CWE_PASSES * CWE_BINS
     cw_evict_state* ev;
+    u32* ev_rank;
     u32 ev_cap;
     // stage 4
     uint8_t* staging;

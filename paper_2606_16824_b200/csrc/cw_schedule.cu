@@ -16,7 +16,7 @@
 namespace {
 
 #define CWS_THREADS 256
-#define CWS_I_PER_CTA 32                      // elements ranked by one CTA
+#define CWS_I_PER_CTA 8                       // elements ranked by one CTA
 #define CWS_J_LANES (CWS_THREADS / CWS_I_PER_CTA)  // threads sharing one element (split the j range)
 #define CWS_TILE 1024                         // keys staged per shared-memory tile
 
@@ -99,9 +99,10 @@ __global__ void __launch_bounds__(CWS_THREADS)
     __syncthreads();
     const u32 per = (R + CWS_THREADS - 1) / CWS_THREADS;
     const u32 lo = min(R, tid * per), hi = min(R, lo + per);
-    const volatile u32* as = a_sorted;  // written by other CTAs: bypass L1
+    // a_sorted was written by other CTAs: read it through L2 (__ldcg), loads independent of one another
     u64 local = 0;
-    for (u32 p = lo; p < hi; ++p) local += as[p];
+#pragma unroll 8
+    for (u32 p = lo; p < hi; ++p) local += __ldcg(a_sorted + p);
     const u32 lane = tid & 31, warp = tid >> 5;
     u64 inc = local;
 #pragma unroll
@@ -125,8 +126,9 @@ __global__ void __launch_bounds__(CWS_THREADS)
     const u64 budget = (u64)free_blocks + (u64)evictable;
     u32 cnt = 0;
     u64 last_need = 0;
+#pragma unroll 8
     for (u32 p = lo; p < hi; ++p) {
-        run += as[p];
+        run += __ldcg(a_sorted + p);
         if (p < max_admit && run <= budget) {  // monotone in p: the admitted set is a prefix
             ++cnt;
             last_need = run;

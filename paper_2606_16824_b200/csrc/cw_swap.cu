@@ -123,10 +123,15 @@ int32_t cwi_copy_pages(cw_ctx* ctx, cudaStream_t stream, const u32* d_ids, const
     a.chunk_bytes = ctx->cfg.chunk_bytes;
     a.chunk_stride = ctx->cfg.chunk_stride;
     a.block_stride = ctx->cfg.block_stride;
+    if (a.chunk_stride == a.chunk_bytes) {  // block-major pool: a page is contiguous, move it as one chunk
+        a.chunk_bytes *= a.n_chunks;
+        a.chunk_stride = a.chunk_bytes;
+        a.n_chunks = 1;
+    }
     a.pieces_per_chunk = (u32)((a.chunk_bytes + CWC_PIECE - 1) / CWC_PIECE);
     a.pool_blocks = ctx->cfg.num_blocks;
     a.status = ctx->d_status;
-    const u64 items = (u64)(cap - first) * a.n_chunks * a.pieces_per_chunk;
+    const u64 items = (u64)(cap - first) * a.n_chunks * a.pieces_per_chunk;  // a.n_chunks: after coalescing
     u64 grid = (u64)ctx->copy_grid;
     if (grid > items) grid = items;
     if (gather)

@@ -148,6 +148,8 @@ __global__ void insert_reset_kernel(cw_slot* table, u32 n, const u32* ins_slot) 
 }
 
 // ---------------------------------------------------------------------------------------------- match
+#define CWM_CHUNK 1024  // consecutive hashes handled by one warp task (32 rounds of 32)
+
 __global__ void __launch_bounds__(256) match_probe_kernel(const cw_slot* __restrict__ table, u64 mask,
                                                           const u64* __restrict__ hashes,
                                                           const u64* __restrict__ hash_off, u32 R, u32* first_miss,
@@ -155,50 +157,73 @@ __global__ void __launch_bounds__(256) match_probe_kernel(const cw_slot* __restr
     const u64 h_first = hash_off[0], total = hash_off[R];  // hash_off may be a slice of a longer CSR array
     const u32 lane = threadIdx.x & 31;
     const u64 nwarps = ((u64)gridDim.x * blockDim.x) >> 5;
-    for (u64 w = ((u64)blockIdx.x * blockDim.x + threadIdx.x) >> 5; h_first + w * 32 < total; w += nwarps) {
-        const u64 g0 = h_first + w * 32, g = g0 + lane;
-        // largest r with hash_off[r] <= g0 (r < R), 32-ary search, warp-uniform
+    // a warp walks its task front to back, so once it has seen a miss of a request the rest of that request is
+    // answered without touching the table (the leading run is over); a miss recorded by an earlier task of the
+    // same request is honoured too when the warp enters that request
+    for (u64 w = ((u64)blockIdx.x * blockDim.x + threadIdx.x) >> 5; h_first + w * CWM_CHUNK < total; w += nwarps) {
+        const u64 c0 = h_first + w * CWM_CHUNK;
+        // largest r with hash_off[r] <= c0 (r < R), 32-ary search, warp-uniform, once per task
         u32 lo = 0, hi = R;
         while (hi - lo > 1) {
             u32 step = (hi - lo + 31) >> 5;
             u32 p = lo + lane * step;
-            bool ok = p < hi && hash_off[p] <= g0;
+            bool ok = p < hi && hash_off[p] <= c0;
             u32 cnt = __popc(__ballot_sync(0xffffffffu, ok));
             u32 nlo = lo + (cnt - 1) * step;
             hi = min(hi, nlo + step);
             lo = nlo;
         }
-        const bool active = g < total;
-        u32 r = lo;
-        u32 loc = CW_MISS;
-        if (active) {
-            while (g >= hash_off[r + 1]) ++r;  // skips empty requests; rare past the first iteration
-            table_find(table, mask, cw_remap_key(hashes[g]), &loc);
-        }
-        const u32 j = active ? (u32)(g - hash_off[r]) : 0;
-        const bool uniform = __all_sync(0xffffffffu, !active || r == lo);
-        const u32 act_mask = __ballot_sync(0xffffffffu, active);
-        if (uniform) {
-            const u32 miss_mask = __ballot_sync(0xffffffffu, active && loc == CW_MISS);
-            const u32 first = miss_mask ? (u32)__ffs(miss_mask) - 1 : 32;
-            const bool behind = lane > first;
-            if (behind) loc = CW_MISS;
-            const u32 hit_mask = act_mask & (first >= 32 ? 0xffffffffu : ((1u << first) - 1));
-            const u32 host_mask = __ballot_sync(0xffffffffu, active && loc != CW_MISS && (loc & CW_HOST_BIT));
-            if (lane == 0 && act_mask) {
-                if (miss_mask) atomicMin(&first_miss[r], j + first);
-                if (hit_mask) atomicMax(&max_hit[r], j + (32 - __clz(hit_mask)));
-                if (host_mask) atomicAdd(&host_hits[r], __popc(host_mask));
+        u32 r_base = lo;  // request of the first hash of the current round (kept up to date below)
+        u32 dead_r = 0xFFFFFFFFu, checked_r = 0xFFFFFFFFu;  // request known to have missed / whose global state was read
+        const u64 c1 = min(total, c0 + CWM_CHUNK);
+        u64 key_next = c0 + lane < c1 ? hashes[c0 + lane] : 0;
+        for (u64 g0 = c0; g0 < c1; g0 += 32) {
+            while (g0 >= hash_off[r_base + 1]) ++r_base;  // warp-uniform; also skips empty requests
+            const u64 g = g0 + lane;
+            const bool active = g < c1;
+            const u64 key = key_next;
+            if (g + 32 < c1) key_next = hashes[g + 32];  // prefetch the next round
+            u32 r = r_base;
+            if (active)
+                while (g >= hash_off[r + 1]) ++r;
+            const u32 j = active ? (u32)(g - hash_off[r]) : 0;
+            const bool uniform = __all_sync(0xffffffffu, !active || r == r_base);
+            const u32 act_mask = __ballot_sync(0xffffffffu, active);
+            if (uniform) {
+                if (r_base != checked_r && r_base != dead_r) {  // entering a request: did an earlier task miss?
+                    checked_r = r_base;
+                    const u32 j0 = (u32)(g0 - hash_off[r_base]);
+                    if (j0 > 0 && __ldcg(first_miss + r_base) < j0) dead_r = r_base;
+                }
+                if (r_base == dead_r) {  // the whole round lies behind a known miss
+                    if (active && hit_loc) hit_loc[g] = CW_MISS;
+                    continue;
+                }
             }
-        } else if (active) {
-            if (loc == CW_MISS) {
-                atomicMin(&first_miss[r], j);
-            } else {
-                atomicMax(&max_hit[r], j + 1);
-                if (loc & CW_HOST_BIT) atomicAdd(&host_hits[r], 1u);
+            u32 loc = CW_MISS;
+            if (active) table_find(table, mask, cw_remap_key(key), &loc);
+            if (uniform) {
+                const u32 miss_mask = __ballot_sync(0xffffffffu, active && loc == CW_MISS);
+                const u32 first = miss_mask ? (u32)__ffs(miss_mask) - 1 : 32;
+                if (lane > first) loc = CW_MISS;
+                const u32 hit_mask = act_mask & (first >= 32 ? 0xffffffffu : ((1u << first) - 1));
+                const u32 host_mask = __ballot_sync(0xffffffffu, active && loc != CW_MISS && (loc & CW_HOST_BIT));
+                if (miss_mask) dead_r = r_base;
+                if (lane == 0) {
+                    if (miss_mask) atomicMin(&first_miss[r], j + first);
+                    if (hit_mask) atomicMax(&max_hit[r], j + (32 - __clz(hit_mask)));
+                    if (host_mask) atomicAdd(&host_hits[r], __popc(host_mask));
+                }
+            } else if (active) {
+                if (loc == CW_MISS) {
+                    atomicMin(&first_miss[r], j);
+                } else {
+                    atomicMax(&max_hit[r], j + 1);
+                    if (loc & CW_HOST_BIT) atomicAdd(&host_hits[r], 1u);
+                }
             }
+            if (active && hit_loc) hit_loc[g] = loc;
         }
-        if (active && hit_loc) hit_loc[g] = loc;
     }
 }
 
@@ -300,7 +325,7 @@ int32_t cwi_match_prefix(cw_ctx* ctx, const u64* d_hashes, const u64* d_hash_off
     if (!R) return CW_OK;
     const u64 mask = ctx->n_slots - 1;
     // enough warps to cover max_hashed_blocks once, capped at a few waves; the kernel grid-strides
-    u64 warps = (ctx->cfg.max_hashed_blocks + 31) / 32;
+    u64 warps = (ctx->cfg.max_hashed_blocks + CWM_CHUNK - 1) / CWM_CHUNK;
     u64 blocks = (warps + 7) / 8;
     u64 cap = (u64)ctx->n_sm * 8 * 4;
     if (blocks > cap) blocks = cap;

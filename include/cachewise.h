@@ -84,6 +84,9 @@ int32_t cw_sync(cw_ctx* ctx);
 int32_t cw_join_copy(cw_ctx* ctx);
 /* Text of the last CW_E_CUDA failure ("" if none).  Valid until the next call on this ctx. */
 const char* cw_last_error(cw_ctx* ctx);
+/* Diagnostics: waits for stream_main, then copies the 32 device timestamps (ns, %globaltimer) that CTA 0 of the
+ * last cw_score_evict took after each of its grid-wide phases; h_out32[31] = how many are valid. */
+int32_t cw_debug_evict_times(cw_ctx* ctx, uint64_t* h_out32);
 /* Number of kernels this ctx has launched so far (bench.py's gpu_launches). */
 uint64_t cw_launch_count(const cw_ctx* ctx);
 

@@ -21,7 +21,7 @@ CW_REF_VALID = 0x80000000
 CW_REF_PINNED = 0x40000000
 POLICY_MIN_ADDITIONAL, POLICY_OVERLAP_FIRST, POLICY_FCFS = 0, 1, 2
 
-EXPORTS = ["cw_create", "cw_destroy", "cw_sync", "cw_join_copy", "cw_last_error", "cw_launch_count", "cw_hash_blocks",
+EXPORTS = ["cw_create", "cw_destroy", "cw_sync", "cw_join_copy", "cw_debug_evict_times", "cw_last_error", "cw_launch_count", "cw_hash_blocks",
            "cw_match_prefix", "cw_schedule", "cw_score_evict", "cw_swap_out", "cw_swap_in", "cw_gather_pages",
            "cw_scatter_pages", "cw_table_insert", "cw_table_erase", "cw_table_retag", "cw_table_lookup",
            "cw_blocks_update"]
@@ -58,6 +58,7 @@ def lib():
         L.cw_destroy.argtypes = [P]
         L.cw_sync.argtypes = [P]
         L.cw_join_copy.argtypes = [P]
+        L.cw_debug_evict_times.argtypes = [P, P]
         L.cw_last_error.argtypes = [P]
         L.cw_last_error.restype = C.c_char_p
         L.cw_launch_count.argtypes = [P]
@@ -138,6 +139,13 @@ class Context:
 
     def join_copy(self):
         self._ck(lib().cw_join_copy(self._h), "cw_join_copy")
+
+    def debug_evict_times(self):
+        """Phase timestamps (ns) of the last score_evict, relative to its first one."""
+        buf = (C.c_uint64 * 32)()
+        self._ck(lib().cw_debug_evict_times(self._h, buf), "cw_debug_evict_times")
+        n = min(int(buf[31]), 31)
+        return [int(buf[i]) - int(buf[0]) for i in range(n)]
 
     @property
     def launches(self):

@@ -1,5 +1,6 @@
 // C-ABI entry points of libcachewise.so: ctx lifetime, host-side argument checks, and the PCIe legs of
 // stage 4.  Every check that needs no device data happens here, before any launch (include/cachewise.h).
+#include <stddef.h>
 #include <stdio.h>
 #include <string.h>
 
@@ -47,7 +48,10 @@ void free_all(cw_ctx* c) {
     cudaFree(c->out_id);
     cudaFree(c->hist);
     cudaFree(c->ev);
-    cudaFree(c->ev_rank);
+    cudaFree(c->ev_bhist);
+    cudaFree(c->ev_boff);
+    cudaFree(c->ev_bcur);
+    cudaFree(c->ev_blist);
     cudaFree(c->staging);
     if (c->own_copy_stream && c->s_copy) cudaStreamDestroy(c->s_copy);
 }
@@ -133,7 +137,10 @@ int32_t cw_create(const cw_config* cfg, cw_ctx** out) {
     CW_CUDA(c, dalloc_zero(&c->out_id, c->ev_cap, s));
     CW_CUDA(c, dalloc_zero(&c->hist, (size_t)CWE_PASSES * CWE_BINS, s));
     CW_CUDA(c, dalloc_zero(&c->ev, 1, s));
-    CW_CUDA(c, dalloc_zero(&c->ev_rank, c->ev_cap, s));
+    CW_CUDA(c, dalloc_zero(&c->ev_bhist, 65536, s));
+    CW_CUDA(c, dalloc_zero(&c->ev_boff, 65537, s));
+    CW_CUDA(c, dalloc_zero(&c->ev_bcur, 65536, s));
+    CW_CUDA(c, dalloc_zero(&c->ev_blist, 196608, s));
     // stage 4
     if (cfg->staging_bytes) {
         if (!cfg->n_chunks || cfg->staging_bytes / 2 < c->page_bytes) {
@@ -179,6 +186,15 @@ int32_t cw_join_copy(cw_ctx* ctx) {
     if (!ctx) return CW_E_STATE;
     CW_CUDA(ctx, cudaEventRecord(ctx->ev_join, ctx->s_copy));
     CW_CUDA(ctx, cudaStreamWaitEvent(ctx->s_main, ctx->ev_join, 0));
+    return CW_OK;
+}
+
+int32_t cw_debug_evict_times(cw_ctx* ctx, uint64_t* h_out32) {
+    if (!ctx) return CW_E_STATE;
+    if (!h_out32) return CW_E_INVAL;
+    CW_CUDA(ctx, cudaStreamSynchronize(ctx->s_main));
+    CW_CUDA(ctx, cudaMemcpy(h_out32, reinterpret_cast<uint8_t*>(ctx->ev) + offsetof(cw_evict_state, stamps),
+                            CWE_STAMPS * sizeof(u64), cudaMemcpyDeviceToHost));
     return CW_OK;
 }
 

@@ -11,12 +11,15 @@
 //      levels when thousands of blocks share tau and age.  Bins below the threshold bin are victims, the
 //      threshold bin becomes the next candidate set; a set of <= 4096 is finished by one CTA in shared memory.
 //      Histograms use warp-aggregated shared-memory atomics (blocks of one session share a digit).
-//   D  victims are sorted by (score, id): 4096-element bitonic runs in shared memory, then a rank merge —
-//      for every (run, tile of victims) a CTA stages the run in shared memory and adds, for each victim of the
-//      tile, the number of smaller keys in that run to the victim's rank.
+//   D  victims are ordered by (score, id): one more split on the top 16 bits that vary among the victims
+//      (65536 buckets: global histogram, scan, scatter), then every bucket is finished on its own — up to 32
+//      keys by one warp (rank counting with shuffles), up to 4096 by one CTA (warp-chunk bitonic + merge-path
+//      rounds in shared memory), anything larger by a grid-wide bitonic network (fallback, adversarial keys only).
+//      An answer of <= 4096 victims is sorted by one CTA directly.
 //   E  scratch is re-zeroed for the next call (the kernel is self-cleaning => graph-capturable)
 // This replaces the paper's eviction heap + rebuild every N_rebuild=3 iterations (L252-254): a full
 // re-score and exact selection per call equals popping a heap rebuilt at this instant.
+#include <stddef.h>
 #include <stdio.h>
 
 #include "cw_internal.cuh"
@@ -25,7 +28,7 @@ namespace {
 
 #define CWE_THREADS 1024
 #define CWE_WARPS (CWE_THREADS / 32)
-#define CWE_ITEMS 2
+#define CWE_ITEMS 4
 #define CWE_TILE (CWE_THREADS * CWE_ITEMS)
 #define CWE_SMEM_SESS 4096                       // sessions whose tau fits the per-CTA shared-memory table
 #define CWE_SMEM_SORT (CWE_SORT_RUN * 24)        // two (score,id) buffers of the CTA sort (alias the histogram)
@@ -50,7 +53,10 @@ struct EvictArgs {
     u32* cand_id[2];
     u64* out_score;
     u32* out_id;
-    u32* rank;       // aliases cand_id[0] (dead once the selection is over)
+    u32* bhist;      // phase D: victims per bucket, exclusive scan, scatter cursors, bucket work lists
+    u32* boff;
+    u32* bcur;
+    u32* blist;
     u32* hist;       // [CWE_PASSES][CWE_BINS]
     cw_evict_state* st;
     u32* status;
@@ -78,28 +84,42 @@ __device__ __forceinline__ void grid_barrier(cw_evict_state* st, u32 nblocks) {
     __syncthreads();
 }
 
+// phase timestamps of the last call (CTA 0 only; read back by cw_debug_evict_times)
+__device__ __forceinline__ void stamp(cw_evict_state* st, u32& n) {
+    if (blockIdx.x == 0 && threadIdx.x == 0 && n < CWE_STAMPS) {
+        u64 t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        st->stamps[n] = t;
+    }
+    ++n;
+}
+
 __device__ __forceinline__ bool key_lt(u64 s1, u32 i1, u64 s2, u32 i2) { return s1 < s2 || (s1 == s2 && i1 < i2); }
 
 // ---- digit plan: up to 11 bit positions of the 96-bit key (95 = MSB of the score, 0 = LSB of the id), descending
+#define CWE_BUCKET_BITS 16                       // digit of the victim bucketing (phase D)
+#define CWE_BUCKETS (1u << CWE_BUCKET_BITS)
 struct DigitPlan {
     u32 nbits;
-    u32 pos[CWE_DIGIT_BITS];
+    u32 pos[CWE_BUCKET_BITS];
 };
 __device__ __forceinline__ u32 key_bit(u64 score, u32 id, u32 pos) {
     return pos >= 32 ? (u32)(score >> (pos - 32)) & 1u : (id >> pos) & 1u;
 }
+template <int MAXBITS = CWE_DIGIT_BITS>
 __device__ __forceinline__ u32 plan_digit(const DigitPlan& pl, u64 score, u32 id) {
     u32 d = 0;
 #pragma unroll
-    for (int i = 0; i < CWE_DIGIT_BITS; ++i)
+    for (int i = 0; i < MAXBITS; ++i)
         if (i < (int)pl.nbits) d = (d << 1) | key_bit(score, id, pl.pos[i]);
     return d;
 }
 // the top 11 set bits of (vary_hi : vary_lo); then, if `fill_from` < 96, contiguous bits from there downwards
-__device__ __forceinline__ void make_plan(DigitPlan* pl, u64 vary_hi, u32 vary_lo, u32 fill_from) {
+__device__ __forceinline__ void make_plan(DigitPlan* pl, u64 vary_hi, u32 vary_lo, u32 fill_from,
+                                          u32 maxbits = CWE_DIGIT_BITS) {
     u32 n = 0;
     u32 lowest = 96;
-    while (n < CWE_DIGIT_BITS && (vary_hi || vary_lo)) {
+    while (n < maxbits && (vary_hi || vary_lo)) {
         u32 p;
         if (vary_hi) {
             p = 63 - __clzll((long long)vary_hi);
@@ -115,7 +135,7 @@ __device__ __forceinline__ void make_plan(DigitPlan* pl, u64 vary_hi, u32 vary_l
     if (fill_from < 96) {
         // plain bits below every chosen one keep the digit a monotone function of the key
         u32 p = lowest == 96 ? fill_from : min(fill_from, lowest - 1);
-        while (n < CWE_DIGIT_BITS) {
+        while (n < maxbits) {
             pl->pos[n++] = p;
             if (p == 0) break;
             --p;
@@ -277,13 +297,14 @@ __device__ __forceinline__ void block_or_to_global(u64 hi, u32 lo, u64* g_hi, u3
 }
 
 // threshold bin of a level: the bin in which the `remaining`-th smallest candidate falls
+template <bool GLOBAL>
 __device__ __forceinline__ void find_threshold(const u32* h, u32 remaining, u32* s_scan, u32* s_thr) {
     constexpr int PER = CWE_BINS / CWE_THREADS;
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     u32 v[PER], sum = 0;
 #pragma unroll
     for (int k = 0; k < PER; ++k) {
-        v[k] = __ldcg(h + tid * PER + k);
+        v[k] = GLOBAL ? __ldcg(h + tid * PER + k) : h[tid * PER + k];
         sum += v[k];
     }
     u32 inc = sum;
@@ -336,12 +357,14 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     __shared__ u32 s_thr[3];  // threshold bin, count before it, count inside it
     __shared__ u64 s_mhi[CWE_WARPS];
     __shared__ u32 s_mlo[CWE_WARPS];
-    __shared__ u64 s_acc_hi;
-    __shared__ u32 s_acc_lo;
+    __shared__ u64 s_acc_hi, s_acc2_hi;
+    __shared__ u32 s_acc_lo, s_acc2_lo, s_cnt[2];
     __shared__ DigitPlan s_plan;
     const u32 tid = threadIdx.x, G = gridDim.x;
     cw_evict_state* st = a.st;
     const bool tau_smem = a.S <= CWE_SMEM_SESS;
+    u32 n_stamp = 0;
+    stamp(st, n_stamp);
 
     // ---------------------------------------------------------------- A: per-session tau
     {
@@ -364,7 +387,10 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
                 tau = min(a.tau_override[s], CW_TAU_MAX - 1);
             } else {
                 i32 raw = a.bias;
-                for (u32 f = 0; f < a.F; ++f) raw += (i32)a.weights[f] * (i32)a.features[(u64)s * a.F + f];
+                const uint8_t* x = a.features + (u64)s * a.F;
+#pragma unroll
+                for (u32 f = 0; f < 16; ++f)  // F <= 16: predicated, independent loads (one latency, not F)
+                    if (f < a.F) raw += (i32)a.weights[f] * (i32)x[f];
                 tau = (u32)min(max(raw, 0), (i32)(CW_TAU_MAX - 1));
             }
             if (tau_smem) s_tau[s] = tau;
@@ -379,6 +405,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
         } else {
             block_or_to_global(packed, 0u, &st->tau_masks, &s_acc_lo, s_mhi, s_mlo);
             grid_barrier(st, G);
+            stamp(st, n_stamp);
             if (tid == 0) s_acc_hi = __ldcg(reinterpret_cast<const unsigned long long*>(&st->tau_masks));
             __syncthreads();
         }
@@ -398,23 +425,29 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
             bool f0[CWE_ITEMS], f1[CWE_ITEMS];
             u32 p0[CWE_ITEMS], p1[CWE_ITEMS];
             u64 sc[CWE_ITEMS];
+            // all four metadata words of every block are loaded up front (independent loads, one latency)
+            u32 rf[CWE_ITEMS], se[CWE_ITEMS], la[CWE_ITEMS], dp[CWE_ITEMS];
+#pragma unroll
+            for (int k = 0; k < CWE_ITEMS; ++k) {
+                const u32 b = tile * CWE_TILE + k * CWE_THREADS + tid;
+                const bool in = b < a.M;
+                rf[k] = in ? a.m_ref[b] : 0u;
+                se[k] = in ? a.m_session[b] : 0u;
+                la[k] = in ? a.m_last[b] : 0u;
+                dp[k] = in ? a.m_depth[b] : 0u;
+            }
 #pragma unroll
             for (int k = 0; k < CWE_ITEMS; ++k) {
                 const u32 b = tile * CWE_TILE + k * CWE_THREADS + tid;
                 f0[k] = false;
                 f1[k] = false;
                 sc[k] = 0;
-                if (b < a.M) {
-                    const u32 rf = a.m_ref[b];
-                    if ((rf & CW_REF_VALID) && !(rf & CW_REF_PINNED) && (rf & 0x3FFFFFFFu) == 0) {
-                        const u32 sess = a.m_session[b];
-                        const u32 tau = sess < a.S ? (tau_smem ? s_tau[sess] : __ldcg(a.tau_q + sess)) : CW_TAU_MAX;
-                        const u32 la = a.m_last[b];
-                        const u32 age = min(a.tick_now >= la ? a.tick_now - la : 0u, 0xFFFFFu);
-                        const u32 dp = min(a.m_depth[b], 0xFFFFFu);
-                        sc[k] = ((u64)(CW_TAU_MAX - tau) << 40) | ((u64)(0xFFFFFu - age) << 20) | (u64)(0xFFFFFu - dp);
-                        f0[k] = true;
-                    }
+                if ((rf[k] & CW_REF_VALID) && !(rf[k] & CW_REF_PINNED) && (rf[k] & 0x3FFFFFFFu) == 0) {
+                    const u32 tau = se[k] < a.S ? (tau_smem ? s_tau[se[k]] : __ldcg(a.tau_q + se[k])) : CW_TAU_MAX;
+                    const u32 age = min(a.tick_now >= la[k] ? a.tick_now - la[k] : 0u, 0xFFFFFu);
+                    const u32 dpc = min(dp[k], 0xFFFFFu);
+                    sc[k] = ((u64)(CW_TAU_MAX - tau) << 40) | ((u64)(0xFFFFFu - age) << 20) | (u64)(0xFFFFFu - dpc);
+                    f0[k] = true;
                 }
                 hist_add(s_hist, f0[k], f0[k] ? plan_digit(pl, sc[k], b) : 0u);
             }
@@ -429,6 +462,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     }
     flush_hist(s_hist, a.hist);
     grid_barrier(st, G);
+    stamp(st, n_stamp);
 
     // ---------------------------------------------------------------- C: radix select
     const u32 n_evictable = __ldcg(&st->n_cand[0]);
@@ -444,29 +478,110 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
         for (int p = 0;; ++p) {
             const u64* cs = a.cand_score[p & 1];
             const u32* ci = a.cand_id[p & 1];
-            if (n_cur <= CWE_SMALL || p >= CWE_PASSES) {
-                // finish in one CTA: sort the candidates, take the first `remaining`
+            if (n_cur <= CWE_LOCAL || p >= CWE_PASSES) {
+                // finish in one CTA, entirely in shared memory: the same radix select without grid barriers,
+                // down to <= 256 candidates, then the `remaining` smallest by rank counting
                 if (blockIdx.x == 0) {
+                    u64 *c_s = s_score, *n_s = t_score;
+                    u32 *c_i = s_id, *n_i = t_id;
+                    u32* l_hist = s_tau;  // the tau table is dead after phase B
                     const u32 base = __ldcg(&st->n_out);
-                    const u32 N = sort_size(min(n_cur, (u32)CWE_SORT_RUN));
+                    u32 emitted = 0, n = n_cur;
+                    u64 v_or_hi = 0, v_nand_hi = 0;
+                    u32 v_or_lo = 0, v_nand_lo = 0;
                     __syncthreads();
-                    for (u32 i = tid; i < N; i += CWE_THREADS) {
-                        s_score[i] = i < n_cur ? __ldcg(cs + i) : ~0ull;
-                        s_id[i] = i < n_cur ? __ldcg(ci + i) : 0xFFFFFFFFu;
+                    for (u32 i = tid; i < n; i += CWE_THREADS) {
+                        c_s[i] = __ldcg(cs + i);
+                        c_i[i] = __ldcg(ci + i);
+                    }
+                    for (;;) {
+                        __syncthreads();
+                        if (n <= CWE_SMALL) {  // 4 threads per candidate
+                            const u32 e = tid >> 2, part = tid & 3;
+                            u32 rank = 0;
+                            u64 ms = 0;
+                            u32 mi = 0;
+                            if (e < n) {
+                                ms = c_s[e];
+                                mi = c_i[e];
+                                for (u32 o = part; o < n; o += 4) rank += key_lt(c_s[o], c_i[o], ms, mi) ? 1u : 0u;
+                            }
+                            rank += __shfl_xor_sync(0xffffffffu, rank, 1);
+                            rank += __shfl_xor_sync(0xffffffffu, rank, 2);
+                            if (e < n && part == 0 && rank < remaining) {
+                                a.out_score[base + emitted + rank] = ms;
+                                a.out_id[base + emitted + rank] = mi;
+                                v_or_hi |= ms;
+                                v_nand_hi |= ~ms;
+                                v_or_lo |= mi;
+                                v_nand_lo |= ~mi;
+                            }
+                            break;
+                        }
+                        // bits that vary inside the current set -> digit plan
+                        u64 o_hi = 0, x_hi = 0;
+                        u32 o_lo = 0, x_lo = 0;
+                        for (u32 i = tid; i < n; i += CWE_THREADS) {
+                            o_hi |= c_s[i];
+                            x_hi |= ~c_s[i];
+                            o_lo |= c_i[i];
+                            x_lo |= ~c_i[i];
+                        }
+                        if (tid == 0) {
+                            s_acc_hi = 0;
+                            s_acc_lo = 0;
+                            s_acc2_hi = 0;
+                            s_acc2_lo = 0;
+                            s_cnt[0] = 0;
+                            s_cnt[1] = 0;
+                        }
+                        for (u32 i = tid; i < CWE_BINS; i += CWE_THREADS) l_hist[i] = 0;
+                        __syncthreads();
+                        block_or_to_global(o_hi, o_lo, &s_acc_hi, &s_acc_lo, s_mhi, s_mlo);
+                        block_or_to_global(x_hi, x_lo, &s_acc2_hi, &s_acc2_lo, s_mhi, s_mlo);
+                        if (tid == 0) make_plan(&s_plan, s_acc_hi & s_acc2_hi, s_acc_lo & s_acc2_lo, 96);
+                        __syncthreads();
+                        const DigitPlan lp = s_plan;
+                        for (u32 i = tid; i < n; i += CWE_THREADS) atomicAdd(&l_hist[plan_digit(lp, c_s[i], c_i[i])], 1u);
+                        __syncthreads();
+                        find_threshold<false>(l_hist, remaining, s_scan, s_thr);
+                        const u32 thr = s_thr[0], before = s_thr[1], inside = s_thr[2];
+                        const u32 need_here = remaining - before;
+                        const bool take_all = need_here == inside;
+                        for (u32 i = tid; i < n; i += CWE_THREADS) {
+                            const u64 ms = c_s[i];
+                            const u32 mi = c_i[i];
+                            const u32 dg = plan_digit(lp, ms, mi);
+                            if (dg < thr || (take_all && dg == thr)) {
+                                const u32 pos = base + emitted + atomicAdd(&s_cnt[0], 1u);
+                                a.out_score[pos] = ms;
+                                a.out_id[pos] = mi;
+                                v_or_hi |= ms;
+                                v_nand_hi |= ~ms;
+                                v_or_lo |= mi;
+                                v_nand_lo |= ~mi;
+                            } else if (dg == thr) {
+                                const u32 pos = atomicAdd(&s_cnt[1], 1u);
+                                n_s[pos] = ms;
+                                n_i[pos] = mi;
+                            }
+                        }
+                        __syncthreads();
+                        if (take_all) break;
+                        emitted += before;
+                        remaining = need_here;
+                        n = inside;
+                        u64* ts_ = c_s; c_s = n_s; n_s = ts_;
+                        u32* ti_ = c_i; c_i = n_i; n_i = ti_;
                     }
                     __syncthreads();
-                    u64* rs;
-                    u32* ri;
-                    cta_sort(s_score, s_id, t_score, t_id, N, rs, ri);
-                    for (u32 i = tid; i < remaining; i += CWE_THREADS) {
-                        a.out_score[base + i] = rs[i];
-                        a.out_id[base + i] = ri[i];
-                    }
+                    block_or_to_global(v_or_hi, v_or_lo, &st->vic_or_hi, &st->vic_or_lo, s_mhi, s_mlo);
+                    block_or_to_global(v_nand_hi, v_nand_lo, &st->vic_nand_hi, &st->vic_nand_lo, s_mhi, s_mlo);
                 }
                 break;
             }
             // threshold bin of this level (every CTA computes it redundantly from the global histogram)
-            find_threshold(a.hist + p * CWE_BINS, remaining, s_scan, s_thr);
+            find_threshold<true>(a.hist + p * CWE_BINS, remaining, s_scan, s_thr);
             const u32 thr = s_thr[0], before = s_thr[1], inside = s_thr[2];
             const u32 need_here = remaining - before;
             const bool take_all = need_here == inside;
@@ -475,8 +590,8 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
             // filter: bins below the threshold are victims, the threshold bin is the next candidate set
             u64* ns = a.cand_score[(p + 1) & 1];
             u32* ni = a.cand_id[(p + 1) & 1];
-            u64 m_or_hi = 0, m_nand_hi = 0;
-            u32 m_or_lo = 0, m_nand_lo = 0;
+            u64 m_or_hi = 0, m_nand_hi = 0, v_or_hi = 0, v_nand_hi = 0;  // next candidate set / victims
+            u32 m_or_lo = 0, m_nand_lo = 0, v_or_lo = 0, v_nand_lo = 0;
             for (u32 tile = blockIdx.x; (u64)tile * CWE_TILE < n_cur; tile += G) {
                 bool f0[CWE_ITEMS], f1[CWE_ITEMS];
                 u32 p0[CWE_ITEMS], p1[CWE_ITEMS];
@@ -492,8 +607,13 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
                         sc[k] = __ldcg(cs + e);
                         id[k] = __ldcg(ci + e);
                         const u32 dg = plan_digit(pl, sc[k], id[k]);
-                        if (dg < thr || (take_all && dg == thr)) f0[k] = true;
-                        else if (dg == thr) {
+                        if (dg < thr || (take_all && dg == thr)) {
+                            f0[k] = true;
+                            v_or_hi |= sc[k];
+                            v_nand_hi |= ~sc[k];
+                            v_or_lo |= id[k];
+                            v_nand_lo |= ~id[k];
+                        } else if (dg == thr) {
                             f1[k] = true;
                             m_or_hi |= sc[k];
                             m_nand_hi |= ~sc[k];
@@ -514,18 +634,21 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
                     }
                 }
             }
-            if (!take_all && inside > CWE_SMALL) {
+            block_or_to_global(v_or_hi, v_or_lo, &st->vic_or_hi, &st->vic_or_lo, s_mhi, s_mlo);
+            block_or_to_global(v_nand_hi, v_nand_lo, &st->vic_nand_hi, &st->vic_nand_lo, s_mhi, s_mlo);
+            if (!take_all && inside > CWE_LOCAL) {
                 block_or_to_global(m_or_hi, m_or_lo, &st->or_hi[p + 1], &st->or_lo[p + 1], s_mhi, s_mlo);
                 block_or_to_global(m_nand_hi, m_nand_lo, &st->nand_hi[p + 1], &st->nand_lo[p + 1], s_mhi, s_mlo);
             }
             grid_barrier(st, G);
+            stamp(st, n_stamp);
             if (take_all) {
                 remaining = 0;
                 break;
             }
             remaining = need_here;
             n_cur = inside;
-            if (n_cur <= CWE_SMALL || p + 1 >= CWE_PASSES) continue;  // finished by one CTA at the top of the loop
+            if (n_cur <= CWE_LOCAL || p + 1 >= CWE_PASSES) continue;  // finished by one CTA at the top of the loop
             // histogram of the next level over the bits that still vary inside the new candidate set
             if (tid == 0) {
                 const u64 vh = __ldcg(reinterpret_cast<const unsigned long long*>(&st->or_hi[p + 1])) &
@@ -547,90 +670,253 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
             }
             flush_hist(s_hist, a.hist + (p + 1) * CWE_BINS);
             grid_barrier(st, G);
+            stamp(st, n_stamp);
         }
     }
     grid_barrier(st, G);
+    stamp(st, n_stamp);
 
     // ---------------------------------------------------------------- E (early): re-zero scratch
-    // (nothing reads hist / the state any more: every CTA carries `want` in registers)
+    // (nothing reads hist / the selection state any more: every CTA carries `want` in registers)
     for (u32 i = blockIdx.x * CWE_THREADS + tid; i < CWE_PASSES * CWE_BINS; i += G * CWE_THREADS) a.hist[i] = 0;
-    if (blockIdx.x == 0) {
+    // bits that vary among the victims -> digit plan of the bucketing (read before CTA 0 clears the masks)
+    if (tid == 0) {
+        const u64 vh = __ldcg(reinterpret_cast<const unsigned long long*>(&st->vic_or_hi)) &
+                       __ldcg(reinterpret_cast<const unsigned long long*>(&st->vic_nand_hi));
+        const u32 vl = __ldcg(&st->vic_or_lo) & __ldcg(&st->vic_nand_lo);
+        make_plan(&s_plan, vh, vl, 96, CWE_BUCKET_BITS);
+    }
+    __syncthreads();
+    if (blockIdx.x == 0) {  // keeps bar_count/bar_gen and the ordering-phase words
         u32* w = reinterpret_cast<u32*>(st);
-        for (u32 i = 2 + tid; i < sizeof(cw_evict_state) / 4; i += CWE_THREADS) w[i] = 0;  // keeps bar_count/bar_gen
+        for (u32 i = 2 + tid; i < offsetof(cw_evict_state, vic_or_hi) / 4; i += CWE_THREADS) w[i] = 0;
+        if (tid == 0) {
+            st->n_medium = 0;
+            st->n_large = 0;
+            st->n_nonempty = 0;
+        }
     }
     if (want == 0) return;
 
-    // ---------------------------------------------------------------- D: sort the victims
-    const u32 n_runs = (want + CWE_SORT_RUN - 1) / CWE_SORT_RUN;
-    for (u32 run = blockIdx.x; run < n_runs; run += G) {
-        const u32 lo = run * CWE_SORT_RUN, len = min((u32)CWE_SORT_RUN, want - lo);
-        const u32 N = sort_size(len);
+    // ---------------------------------------------------------------- D: order the victims by (score, id)
+    if (want <= CWE_SORT_RUN) {  // small answer: one CTA sorts it (no further grid barrier)
+        if (blockIdx.x == 0) {
+            const u32 N = sort_size(want);
+            __syncthreads();
+            for (u32 i = tid; i < N; i += CWE_THREADS) {
+                s_score[i] = i < want ? __ldcg(a.out_score + i) : ~0ull;
+                s_id[i] = i < want ? __ldcg(a.out_id + i) : 0xFFFFFFFFu;
+            }
+            __syncthreads();
+            u64* rs;
+            u32* ri;
+            cta_sort(s_score, s_id, t_score, t_id, N, rs, ri);
+            for (u32 i = tid; i < want; i += CWE_THREADS) {
+                a.victims[i] = ri[i];
+                if (a.victim_scores) a.victim_scores[i] = rs[i];
+            }
+            stamp(st, n_stamp);
+            if (tid == 0) {  // the masks were only needed for the bucketed path
+                st->stamps[CWE_STAMPS - 1] = n_stamp;
+                st->vic_or_hi = 0;
+                st->vic_nand_hi = 0;
+                st->vic_or_lo = 0;
+                st->vic_nand_lo = 0;
+            }
+        }
+        return;
+    }
+    // D1: bucket = the top 16 bits that vary among the victims (a monotone function of the key), histogram
+    const DigitPlan bp = s_plan;
+    for (u32 e = blockIdx.x * CWE_THREADS + tid; e < want; e += G * CWE_THREADS)
+        atomicAdd(&a.bhist[plan_digit<CWE_BUCKET_BITS>(bp, __ldcg(a.out_score + e), __ldcg(a.out_id + e))], 1u);
+    grid_barrier(st, G);
+    stamp(st, n_stamp);
+    // D2: exclusive scan of the bucket sizes, every CTA on its own slice of 512 buckets: the offset of the slice
+    //     is the sum of all earlier buckets (re-read from L2: at most 256 KiB), so no CTA waits for another
+    {
+        constexpr u32 SLICE = 512;
+        const u32 lane = tid & 31, warp = tid >> 5;
+        for (u32 sl = blockIdx.x; sl < CWE_BUCKETS / SLICE; sl += G) {
+            const u32 first = sl * SLICE;
+            u32 before = 0;
+            for (u32 b = tid * 4; b < first; b += CWE_THREADS * 4) {
+                const uint4 v = __ldcg(reinterpret_cast<const uint4*>(a.bhist + b));
+                before += v.x + v.y + v.z + v.w;
+            }
+            const u32 mine = tid < SLICE ? __ldcg(a.bhist + first + tid) : 0u;
+            // block scan of (before: plain sum, mine: inclusive prefix over tid)
+            u32 inc = mine, tot = before;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                u32 y = __shfl_up_sync(0xffffffffu, inc, d);
+                if (lane >= d) inc += y;
+                tot += __shfl_xor_sync(0xffffffffu, tot, d);
+            }
+            __syncthreads();
+            if (lane == 31) s_scan[warp] = inc;
+            if (lane == 0) s_w0[warp] = tot;
+            __syncthreads();
+            if (warp == 0) {
+                u32 w = s_scan[lane], wi = w, t2 = s_w0[lane];
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    u32 y = __shfl_up_sync(0xffffffffu, wi, d);
+                    if (lane >= d) wi += y;
+                    t2 += __shfl_xor_sync(0xffffffffu, t2, d);
+                }
+                s_scan[lane] = wi - w;
+                if (lane == 0) s_base[0] = t2;
+            }
+            __syncthreads();
+            if (tid < SLICE) {
+                const u32 off = s_base[0] + s_scan[warp] + inc - mine;
+                a.boff[first + tid] = off;
+                a.bcur[first + tid] = off;
+            }
+            // compact list of the non-empty buckets (order irrelevant): one atomic per warp
+            const u32 ne = __ballot_sync(0xffffffffu, mine != 0);
+            u32 lbase = 0;
+            if (lane == 0 && ne) lbase = atomicAdd(&st->n_nonempty, (u32)__popc(ne));
+            lbase = __shfl_sync(0xffffffffu, lbase, 0);
+            if (mine != 0) a.blist[2 * CWE_BUCKETS + lbase + __popc(ne & ((1u << lane) - 1))] = first + tid;
+        }
+        if (blockIdx.x == 0 && tid == 0) {
+            a.boff[CWE_BUCKETS] = want;
+            st->vic_or_hi = 0;
+            st->vic_nand_hi = 0;
+            st->vic_or_lo = 0;
+            st->vic_nand_lo = 0;
+        }
+    }
+    grid_barrier(st, G);
+    stamp(st, n_stamp);
+    // D3: scatter into bucket order (inside a bucket the order is arbitrary for now)
+    u64* tmp_score = a.cand_score[0];
+    u32* tmp_id = a.cand_id[0];
+    for (u32 e = blockIdx.x * CWE_THREADS + tid; e < want; e += G * CWE_THREADS) {
+        const u64 sc = __ldcg(a.out_score + e);
+        const u32 id = __ldcg(a.out_id + e);
+        const u32 pos = atomicAdd(&a.bcur[plan_digit<CWE_BUCKET_BITS>(bp, sc, id)], 1u);
+        tmp_score[pos] = sc;
+        tmp_id[pos] = id;
+    }
+    grid_barrier(st, G);
+    stamp(st, n_stamp);
+    // D4: one warp per bucket: up to 128 keys are sorted by the warp in its own shared-memory chunk (bitonic,
+    //     __syncwarp only) and written to their final place; larger buckets are queued for a CTA sort
+    //     (<= 4096) or the grid-wide fallback
+    {
+        const u32 lane = tid & 31, warp = tid >> 5;
+        u64* ws = s_score + warp * 128;
+        u32* wi = s_id + warp * 128;
+        const u32 gw = (blockIdx.x * CWE_THREADS + tid) >> 5, nw = (G * CWE_THREADS) >> 5;
+        const u32 n_nonempty = __ldcg(&st->n_nonempty);
+        {
+          for (u32 q = gw; q < n_nonempty; q += nw) {
+            const u32 d = __ldcg(a.blist + 2 * CWE_BUCKETS + q);
+            const u32 b0 = __ldcg(a.boff + d), n = __ldcg(a.boff + d + 1) - b0;
+            if (lane == 0) a.bhist[d] = 0;  // self-cleaning
+            if (n == 1) {
+                if (lane == 0) {
+                    a.victims[b0] = __ldcg(tmp_id + b0);
+                    if (a.victim_scores) a.victim_scores[b0] = __ldcg(tmp_score + b0);
+                }
+            } else if (n <= 128) {
+                u32 N = 2;
+                while (N < n) N <<= 1;
+                __syncwarp();
+                for (u32 i = lane; i < N; i += 32) {
+                    ws[i] = i < n ? __ldcg(tmp_score + b0 + i) : ~0ull;
+                    wi[i] = i < n ? __ldcg(tmp_id + b0 + i) : 0xFFFFFFFFu;
+                }
+                __syncwarp();
+                for (u32 k = 2; k <= N; k <<= 1) {
+                    for (u32 j = k >> 1; j > 0; j >>= 1) {
+                        for (u32 t = lane; t < (N >> 1); t += 32) {
+                            const u32 i = ((t & ~(j - 1)) << 1) | (t & (j - 1));
+                            const u32 p = i | j;
+                            const bool up = (i & k) == 0;
+                            const u64 xs = ws[i], ys = ws[p];
+                            const u32 xi = wi[i], yi = wi[p];
+                            if (key_lt(ys, yi, xs, xi) == up) {
+                                ws[i] = ys; wi[i] = yi;
+                                ws[p] = xs; wi[p] = xi;
+                            }
+                        }
+                        __syncwarp();
+                    }
+                }
+                for (u32 i = lane; i < n; i += 32) {
+                    a.victims[b0 + i] = wi[i];
+                    if (a.victim_scores) a.victim_scores[b0 + i] = ws[i];
+                }
+            } else if (lane == 0) {
+                if (n <= CWE_SORT_RUN) a.blist[atomicAdd(&st->n_medium, 1u)] = d;
+                else a.blist[CWE_BUCKETS + atomicAdd(&st->n_large, 1u)] = d;
+            }
+          }
+        }
+    }
+    grid_barrier(st, G);
+    stamp(st, n_stamp);
+    // D5: medium buckets, one CTA each
+    const u32 n_medium = __ldcg(&st->n_medium), n_large = __ldcg(&st->n_large);
+    for (u32 m = blockIdx.x; m < n_medium; m += G) {
+        const u32 d = __ldcg(a.blist + m);
+        const u32 b0 = __ldcg(a.boff + d), n = __ldcg(a.boff + d + 1) - b0;
+        const u32 N = sort_size(n);
         __syncthreads();
         for (u32 i = tid; i < N; i += CWE_THREADS) {
-            s_score[i] = i < len ? __ldcg(a.out_score + lo + i) : ~0ull;
-            s_id[i] = i < len ? __ldcg(a.out_id + lo + i) : 0xFFFFFFFFu;
+            s_score[i] = i < n ? __ldcg(tmp_score + b0 + i) : ~0ull;
+            s_id[i] = i < n ? __ldcg(tmp_id + b0 + i) : 0xFFFFFFFFu;
         }
         __syncthreads();
         u64* rs;
         u32* ri;
         cta_sort(s_score, s_id, t_score, t_id, N, rs, ri);
-        if (n_runs == 1) {
-            for (u32 i = tid; i < len; i += CWE_THREADS) {
-                a.victims[i] = ri[i];
-                if (a.victim_scores) a.victim_scores[i] = rs[i];
-            }
-        } else {
-            for (u32 i = tid; i < len; i += CWE_THREADS) {
-                a.out_score[lo + i] = rs[i];
-                a.out_id[lo + i] = ri[i];
-                a.rank[lo + i] = i;  // rank inside its own run; the other runs are added below
-            }
+        for (u32 i = tid; i < n; i += CWE_THREADS) {
+            a.victims[b0 + i] = ri[i];
+            if (a.victim_scores) a.victim_scores[b0 + i] = rs[i];
         }
     }
-    if (n_runs == 1) return;
-    grid_barrier(st, G);
-
-    // rank merge: item = (run r staged in shared memory, tile of victims searched in it)
-    {
-        const u64 work = (u64)want * n_runs;
-        u32 tile_e = (u32)((work + 2ull * G - 1) / (2ull * G));
-        tile_e = max(tile_e, (u32)CWE_THREADS);
-        const u32 tiles = (want + tile_e - 1) / tile_e;
-        const u32 items = n_runs * tiles;
-        u32 staged = 0xFFFFFFFFu;
-        for (u32 item = blockIdx.x; item < items; item += G) {
-            const u32 r = item / tiles, t = item - r * tiles;
-            const u32 lo = r * CWE_SORT_RUN, len = min((u32)CWE_SORT_RUN, want - lo);
-            if (staged != r) {
-                __syncthreads();
-                for (u32 i = tid; i < len; i += CWE_THREADS) {
-                    s_score[i] = __ldcg(a.out_score + lo + i);
-                    s_id[i] = __ldcg(a.out_id + lo + i);
+    // D6: fallback for a bucket of more than 4096 keys (only when the keys defeat the 16-bit split): bitonic
+    //     network for arbitrary n (flip + disperse; partners beyond n count as +inf) in global memory, one grid
+    //     barrier per stage
+    for (u32 l = 0; l < n_large; ++l) {
+        const u32 d = __ldcg(a.blist + CWE_BUCKETS + l);
+        const u32 b0 = __ldcg(a.boff + d), n = __ldcg(a.boff + d + 1) - b0;
+        u64* ks = tmp_score + b0;
+        u32* ki = tmp_id + b0;
+        u32 n_pad = 2;
+        while (n_pad < n) n_pad <<= 1;
+        for (u32 k = 2; k <= n_pad; k <<= 1) {
+            for (u32 j = k >> 1; j > 0; j >>= 1) {
+                const bool flip = j == (k >> 1);  // first stage of a merge: mirror inside the k-block
+                for (u32 t = blockIdx.x * CWE_THREADS + tid; t < (n_pad >> 1); t += G * CWE_THREADS) {
+                    const u32 i = ((t & ~(j - 1)) << 1) | (t & (j - 1));  // lower element of the t-th pair
+                    const u32 partner = flip ? ((i & ~(k - 1)) | ((k - 1) - (i & (k - 1)))) : i + j;
+                    if (partner < n) {  // i < partner; a partner beyond n is +inf: nothing to do
+                        const u64 xs = __ldcg(ks + i), ys = __ldcg(ks + partner);
+                        const u32 xi = __ldcg(ki + i), yi = __ldcg(ki + partner);
+                        if (key_lt(ys, yi, xs, xi)) {
+                            ks[i] = ys; ki[i] = yi;
+                            ks[partner] = xs; ki[partner] = xi;
+                        }
+                    }
                 }
-                __syncthreads();
-                staged = r;
-            }
-            const u32 e0 = t * tile_e, e1 = min(want, e0 + tile_e);
-            for (u32 e = e0 + tid; e < e1; e += CWE_THREADS) {
-                if (e >= lo && e < lo + len) continue;  // its own run
-                const u64 s = __ldcg(a.out_score + e);
-                const u32 id = __ldcg(a.out_id + e);
-                u32 l = 0, h = len;  // number of keys of run r below (s,id)
-                while (l < h) {
-                    const u32 m = (l + h) >> 1;
-                    if (key_lt(s_score[m], s_id[m], s, id)) l = m + 1;
-                    else h = m;
-                }
-                if (l) atomicAdd(&a.rank[e], l);
+                grid_barrier(st, G);
+                stamp(st, n_stamp);
             }
         }
+        for (u32 i = blockIdx.x * CWE_THREADS + tid; i < n; i += G * CWE_THREADS) {
+            a.victims[b0 + i] = __ldcg(ki + i);
+            if (a.victim_scores) a.victim_scores[b0 + i] = __ldcg(ks + i);
+        }
     }
-    grid_barrier(st, G);
-    for (u32 e = blockIdx.x * CWE_THREADS + tid; e < want; e += G * CWE_THREADS) {
-        const u32 rk = __ldcg(a.rank + e);
-        a.victims[rk] = __ldcg(a.out_id + e);
-        if (a.victim_scores) a.victim_scores[rk] = __ldcg(a.out_score + e);
-    }
+    __syncthreads();
+    stamp(st, n_stamp);
+    if (blockIdx.x == 0 && tid == 0) st->stamps[CWE_STAMPS - 1] = n_stamp;
 }
 
 int g_evict_grid = 0;
@@ -673,7 +959,10 @@ int32_t cwi_score_evict(cw_ctx* ctx, u32 tick_now, u32 S, u32 F, const uint8_t* 
     a.cand_id[1] = ctx->cand_id[1];
     a.out_score = ctx->out_score;
     a.out_id = ctx->out_id;
-    a.rank = ctx->ev_rank;
+    a.bhist = ctx->ev_bhist;
+    a.boff = ctx->ev_boff;
+    a.bcur = ctx->ev_bcur;
+    a.blist = ctx->ev_blist;
     a.hist = ctx->hist;
     a.st = ctx->ev;
     a.status = ctx->d_status;

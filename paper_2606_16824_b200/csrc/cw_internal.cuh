@@ -77,7 +77,9 @@ struct cw_hash_rec {  // what the CTA of one range publishes for the CTA of the 
 #define CWE_BINS 2048          // 11-bit digits
 #define CWE_DIGIT_BITS 11
 #define CWE_PASSES 12          // level 0 (tau bits) + at most ceil(96/11) levels over bits that still vary
-#define CWE_SMALL 4096         // finish in one CTA when the candidate set is this small
+#define CWE_STAMPS 32
+#define CWE_LOCAL 4096         // a candidate set this small is finished by one CTA in shared memory ...
+#define CWE_SMALL 256          // ... by radix levels down to this size, then rank counting
 #define CWE_SORT_RUN 4096      // victims sorted in runs of this size, then rank-merged
 
 struct cw_evict_state {  // all zero between calls, except the barrier words
@@ -89,6 +91,12 @@ struct cw_evict_state {  // all zero between calls, except the barrier words
     u32 pad1;
     u32 or_lo[CWE_PASSES + 1], nand_lo[CWE_PASSES + 1];  // OR of the ids / of their complements, per level
     u64 or_hi[CWE_PASSES + 1], nand_hi[CWE_PASSES + 1];  // same for the scores
+    // ---- not covered by the early re-zeroing (used by the ordering phase)
+    u64 vic_or_hi, vic_nand_hi;       // OR of the victims' scores / of their complements
+    u32 vic_or_lo, vic_nand_lo;       // same for the ids
+    u32 n_medium, n_large;            // buckets that need a CTA sort / the grid-wide fallback
+    u32 n_nonempty, pad2;             // non-empty buckets
+    u64 stamps[CWE_STAMPS];           // %globaltimer of CTA 0 after every grid barrier; [last] = how many
 };
 
 struct cw_ctx {
@@ -130,7 +138,10 @@ struct cw_ctx {
     u32* out_id;
     u32* hist;  // CWE_PASSES * CWE_BINS
     cw_evict_state* ev;
-    u32* ev_rank;
+    u32* ev_bhist;   // victims per bucket (CWE_BUCKETS)
+    u32* ev_boff;    // exclusive scan (CWE_BUCKETS + 1)
+    u32* ev_bcur;    // scatter cursors (CWE_BUCKETS)
+    u32* ev_blist;   // [0, 65536): medium buckets, [65536, 131072): large, [131072, 196608): non-empty
     u32 ev_cap;
     // stage 4
     uint8_t* staging;

@@ -119,6 +119,59 @@ def test_score_evict_scaled_stress_snapshot_and_host_tier():
     ctx.close()
 
 
+@pytest.mark.parametrize("bulks", [(10000,), (3000, 3000), (5000, 40, 4500)])
+def test_score_evict_ordering_paths_medium_and_large_buckets(bulks):
+    """Keys built to defeat the 16-bit bucket split of the ordering phase: 16 - log2(#bulks) outlier sessions
+    own the top varying bits, so every bulk session (equal tau, thousands of blocks) lands in ONE bucket —
+    medium buckets (CTA sort) and buckets above 4096 keys (grid-wide bitonic fallback) must both agree with
+    the oracle, and so must a repeat of the call (self-cleaning scratch)."""
+    from gpu_util import small_ctx
+    g = gen.rng(33, sum(bulks))
+    nb = len(bulks)
+    low = {1: 0, 2: 1, 3: 2}[nb]                      # tau bits used to tell the bulks apart
+    n_out = 16 - low
+    S = nb + n_out
+    tau = np.zeros(S, np.uint32)
+    for b in range(nb):
+        tau[b] = TAU_MAX - 1 - (b << 8)               # v = TAU_MAX - tau = 1 + (b << 8)
+    for o in range(n_out):
+        tau[nb + o] = TAU_MAX - 1 - (1 << (8 + low + o))
+    sess = np.concatenate([np.full(n, b, np.uint32) for b, n in enumerate(bulks)] +
+                          [np.arange(nb, S, dtype=np.uint32)])
+    M = sess.size
+    perm = g.permutation(M)
+    sess = sess[perm]
+    depth = g.integers(0, 6000, size=M).astype(np.uint32)        # ties inside a bulk: the id decides
+    last = np.full(M, 500, np.uint32)
+    rf = np.full(M, V, np.uint32)
+    feats = np.zeros((S, 4), np.uint8)
+    w = np.zeros(4, np.int16)
+    state = np.zeros(S, np.uint8)
+    ctx = small_ctx(num_blocks=M, table_log2_slots=max(4, int(np.ceil(np.log2(2 * M)))), max_sessions=S)
+    _load_meta(ctx, 0, sess, last, depth, rf)
+    for deficit in (M, M - 7, 4097):
+        ev, es, est = oracle.score_evict(1000, feats, w, 0, state, tau, deficit, sess, last, depth, rf, cap=M)
+        for _ in range(2):
+            gv, gs, gst = _evict(ctx, 1000, feats, w, 0, state, tau, deficit, M)
+            assert gst == est == 0 and gv.tolist() == ev.tolist() and gs.tolist() == es.tolist(), deficit
+    ctx.close()
+
+
+def test_score_evict_more_sessions_than_the_shared_memory_table():
+    """S > 4096: tau goes through global memory (one more grid barrier) instead of the per-CTA table."""
+    from gpu_util import small_ctx
+    g = gen.rng(34, 0)
+    M, S, F = 60000, 5000, 8
+    ctx = small_ctx(num_blocks=M, table_log2_slots=17, max_sessions=S)
+    sess, last, depth, rf, feats, w, state = _random_pool(g, M, S, F)
+    _load_meta(ctx, 0, sess, last, depth, rf)
+    for deficit in (100, 5000, 30000):
+        ev, es, est = oracle.score_evict(1000, feats, w, 500, state, None, deficit, sess, last, depth, rf, cap=M)
+        gv, gs, gst = _evict(ctx, 1000, feats, w, 500, state, None, deficit, M)
+        assert gst == est and gv.tolist() == ev.tolist() and gs.tolist() == es.tolist(), deficit
+    ctx.close()
+
+
 def test_score_evict_host_side_argument_checks():
     import paper_2606_16824_b200 as cw
     from gpu_util import dev, small_ctx, zeros

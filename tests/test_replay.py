@@ -1,0 +1,122 @@
+"""Host-driven replay (R6).
+
+CPU part (`-m "not gpu"`): the shared driver on the oracle backend — invariants that hold for any correct
+backend (every turn completes, capacity is never exceeded, the run is a pure function of the seed, the pool
+bytes of the tiny config equal a scalar re-derivation), plus policy sanity (ground-truth tau
+never evicts more than a constant predictor = LRU on this trace).
+GPU part (`-m gpu`): the CUDA path through the C ABI must reproduce the oracle's replay log element by
+element — hashes, overlap lengths, queue order, admission, victims + scores, staged KV bytes, eviction / drop /
+swap-in counts — on BASELINE.json configs[0] exactly and on configs[1] / configs[4] at reduced session counts
+(same page shapes), where KV bytes are checked on sampled victims against the procedural page content.
+"""
+import numpy as np
+import pytest
+
+from harness import gen, replay
+from oracle.backend import OracleBackend
+
+
+def tiny_cfg(**kw):
+    a = dict(name="configs[0]", num_blocks=256, host_slots=64, n_chunks=4, chunk_bytes=4096, max_admit=2)
+    a.update(kw)
+    return replay.ReplayConfig(**a)
+
+
+def test_tiny_replay_invariants_on_the_oracle():
+    tr = gen.tiny_trace(0)
+    cfg = tiny_cfg()
+    be = OracleBackend(cfg, 4, 4)
+    r = replay.run(tr, cfg, be)
+    assert r.completed == 32 and r.evictions > 0
+    for st in r.steps:
+        assert st.victims.size == np.unique(st.victims).size                  # a block is evicted at most once per step
+        assert st.num_admit <= cfg.max_admit and len(st.admitted) <= max(st.num_admit, 1)
+    # the run is a pure function of (config, seed)
+    r2 = replay.run(gen.tiny_trace(0), cfg, OracleBackend(cfg, 4, 4))
+    assert replay.compare(r, r2) == []
+    # resident HBM pages hold exactly the procedural content of their hash (prefill -> swap round trips)
+    m = be.meta[0]
+    valid = np.nonzero(m["ref_flags"] & 0x80000000)[0]
+    assert valid.size > 0
+    pool = be.read_pool().reshape(cfg.num_blocks, cfg.page)
+    # the table is the ground truth for which hash lives where
+    allh = np.concatenate([s[-1].tokens for s in tr.sessions])
+    for s, turns in enumerate(tr.sessions):
+        h, ho = __import__("oracle").hash_blocks(turns[-1].tokens, [0, turns[-1].tokens.size])
+        loc = be.table.lookup(h)
+        for j in np.nonzero((loc != 0xFFFFFFFF) & ((loc & 0x80000000) == 0))[0][:8]:
+            assert np.array_equal(pool[int(loc[j])], gen.page_bytes(h[j:j + 1], cfg.page)[0])
+
+
+@pytest.mark.parametrize("kw", [dict(), dict(layout="layer", policy=1), dict(num_blocks=160, host_slots=48),
+                                dict(num_blocks=160, host_slots=0), dict(num_blocks=128, host_slots=256, use_hint=True)])
+def test_tiny_variants_complete_and_respect_capacity(kw):
+    tr = gen.tiny_trace(0)
+    cfg = tiny_cfg(**kw)
+    r = replay.run(tr, cfg, OracleBackend(cfg, 4, 4))
+    assert r.completed == 32
+    assert r.hit_blocks + r.new_blocks == sum((t.tokens.size + 15) // 16 for s in tr.sessions for t in s)
+    if cfg.host_slots == 0:
+        assert r.drops == r.evictions and r.swap_ins == 0
+
+
+def test_ground_truth_tau_does_not_evict_more_than_lru():
+    """with the true time-to-next-reuse the policy is Belady's; a constant predictor is LRU."""
+    tr = gen.session_trace(11, 12, 10, 4, 768, 64, 256, 1.0, 1 << 30, [(0.7, 300.0, 1.0), (0.3, 20000.0, 1.0)])
+    flat = gen.Trace(tr.sessions, np.zeros(4, np.int16), 1000, 4, tr.meta)     # every prediction equal -> LRU
+    base = dict(num_blocks=420, host_slots=0, n_chunks=1, chunk_bytes=16, max_admit=4, store_bytes=False)
+    lru = replay.run(flat, replay.ReplayConfig("lru", **base), OracleBackend(replay.ReplayConfig("lru", **base), 12, 4))
+    cfg = replay.ReplayConfig("hint", use_hint=True, **base)
+    hint = replay.run(tr, cfg, OracleBackend(cfg, 12, 4))
+    assert hint.completed == lru.completed == 120
+    assert hint.new_blocks <= lru.new_blocks        # fewer blocks recomputed = fewer harmful evictions
+
+
+# ---------------------------------------------------------------------------------------------- GPU parity
+def _both(tr, cfg, S, F, verify_pages=0):
+    ro = replay.run(tr, cfg, OracleBackend(cfg, S, F))
+    gb = replay.GpuBackend(cfg, S, F, verify_pages=verify_pages)
+    rg = replay.run(tr, cfg, gb)
+    return ro, rg, gb
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("kw", [dict(), dict(layout="layer", policy=1), dict(num_blocks=160, host_slots=48),
+                                dict(num_blocks=128, host_slots=256, use_hint=True, max_admit=3)])
+def test_gpu_tiny_replay_is_bit_exact(kw):
+    tr = gen.tiny_trace(0)
+    cfg = tiny_cfg(**kw)
+    ro, rg, gb = _both(tr, cfg, 4, 4)
+    assert replay.compare(ro, rg) == []
+    assert ro.totals() == rg.totals() and rg.evictions > 0
+    ob = OracleBackend(cfg, 4, 4)
+    replay.run(tr, cfg, ob)
+    assert np.array_equal(gb.read_pool(), ob.read_pool()), "final pool bytes"
+    gb.close()
+
+
+@pytest.mark.gpu
+def test_gpu_llama8b_shaped_replay_reduced():
+    """configs[1] page shape (64 x 32 KiB = 2 MiB, layer-major), pool = 60% of the working set; 6 sessions x 6
+    turns so that the oracle side and the pinned host tier stay small."""
+    tr = gen.llama8b_trace(1, n_sessions=6, n_turns=6)
+    need = sum(max((t.tokens.size + 15) // 16 for t in s) for s in tr.sessions)
+    cfg = replay.ReplayConfig("configs[1]/reduced", int(0.6 * need), need // 2, 64, 32768, layout="layer", max_admit=4,
+                              store_bytes=False)
+    ro, rg, gb = _both(tr, cfg, 6, 8, verify_pages=2)
+    assert replay.compare(ro, rg) == []
+    assert rg.evictions > 0 and rg.swap_ins > 0 and gb.pages_verified > 0
+    gb.close()
+
+
+@pytest.mark.gpu
+def test_gpu_long_agent_replay_reduced():
+    """configs[4] page shape (56 x 16 KiB = 896 KiB), bimodal gaps; 24 sessions x 16 turns growing to 24k tokens."""
+    tr = gen.long_agent_trace(5, n_sessions=24, n_turns=16, cap=24000)
+    need = sum(max((t.tokens.size + 15) // 16 for t in s) for s in tr.sessions)
+    cfg = replay.ReplayConfig("configs[4]/reduced", int(0.5 * need), need // 4, 56, 16384, layout="block", max_admit=8,
+                              store_bytes=False)
+    ro, rg, gb = _both(tr, cfg, 24, 8, verify_pages=1)
+    assert replay.compare(ro, rg) == []
+    assert rg.evictions > 0 and rg.drops > 0 and gb.pages_verified > 0
+    gb.close()

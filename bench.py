@@ -35,9 +35,9 @@ WORKLOAD = ("BASELINE.json configs[2]: 4096 queued requests, 256 sessions x 1310
 PCIE_GEN5_X16_GBS = 63.0  # 32 GT/s x 16 lanes x 128/130 / 8 per direction
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
-# (profiles/r1_full_*.md); None until a capture of that kernel exists.
-NCU_TRAFFIC_BYTES = {"hash": None, "match": None, "score_evict": None, "gather": None, "scatter": None,
-                     "schedule": None}
+# (profiles/r1_full_step_kernels.md), full-size configs[2] step.
+NCU_TRAFFIC_BYTES = {"hash": 433_265_408, "match": 103_412_224, "score_evict": 17_190_400, "gather": 1_660_707_072,
+                     "scatter": 1_660_303_616, "schedule": 105_216}
 
 
 def measured_peaks():
@@ -356,7 +356,7 @@ def run_cuda(args):
         if name in stage_ms and stage_ms[name] > 0:
             ach = alg[name] / stage_ms[name] / 1e6
             rooflines[name] = {"bound": "hbm", "achieved": round(ach, 1), "peak": hbm_peak, "unit": "GB/s",
-                               "frac": round(ach / hbm_peak, 4), "traffic": NCU_TRAFFIC_BYTES.get(name),
+                               "frac": round(ach / hbm_peak, 4), "traffic": NCU_TRAFFIC_BYTES.get(name) if args.scale <= 1 else None,
                                "algorithmic_bytes": alg[name], "us": round(stage_ms[name] * 1e3, 2)}
     dominant = max(stage_ms, key=stage_ms.get)
     roofline = dict(rooflines[dominant], kernel=dominant, peak_source=peak_src)

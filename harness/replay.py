@@ -528,3 +528,58 @@ class GpuBackend:
     def close(self):
         self.ctx.close()
         self.pool = self.tier = None
+
+
+# --------------------------------------------------------------------------------------------------
+# Full-size configurations (BASELINE.json configs[0], [1], [4]) scaled to the box by rule
+# --------------------------------------------------------------------------------------------------
+def full_config(which: int, hbm_budget_gib: float = 120.0, host_budget_gib: float = 48.0, scale: int = 1):
+    """Returns (trace, cfg, note).  Pools are sized by the config's rule, then capped by the memory budgets
+    (page count shrinks, page size never does); the applied scale is stated in `note`."""
+    if which == 0:
+        return gen.tiny_trace(0), ReplayConfig("configs[0]", 256, 64, 4, 4096, max_admit=2), "as specified"
+    if which == 1:
+        tr = gen.llama8b_trace(1, n_sessions=64 // scale, n_turns=40)
+        n_chunks, chunk = 64, 32768
+        frac, max_admit = 0.6, 8
+    elif which == 4:
+        tr = gen.long_agent_trace(5, n_sessions=512 // scale, n_turns=200 // scale, cap=200_000)
+        n_chunks, chunk = 56, 16384
+        frac, max_admit = None, 16
+    else:
+        raise ValueError("replay configs are 0, 1 and 4")
+    page = n_chunks * chunk
+    ws = sum(max((t.tokens.size + 15) // 16 for t in s) for s in tr.sessions)
+    want_m = int(frac * ws) if frac else int(120e9 // page)
+    want_h = ws if which == 1 else int(512e9 // page)
+    m = min(want_m, int(hbm_budget_gib * 2**30 // page))
+    h = min(want_h, int(host_budget_gib * 2**30 // page))
+    note = (f"working set {ws} blocks; pool {m} of {want_m} blocks ({m * page / 2**30:.1f} GiB), host tier {h} of {want_h} "
+            f"slots ({h * page / 2**30:.1f} GiB); sessions/turns scale 1/{scale}")
+    cfg = ReplayConfig(f"configs[{which}]", m, h, n_chunks, chunk, layout="layer" if which == 1 else "block",
+                       max_admit=max_admit, store_bytes=False)
+    return tr, cfg, note
+
+
+def main():
+    import argparse
+    import json
+    import time
+    ap = argparse.ArgumentParser(description="host-driven replay on the CUDA path")
+    ap.add_argument("--config", type=int, default=0, choices=[0, 1, 4])
+    ap.add_argument("--scale", type=int, default=1, help="divide the number of sessions (and turns of config 4)")
+    ap.add_argument("--hbm-gib", type=float, default=120.0)
+    ap.add_argument("--host-gib", type=float, default=48.0)
+    a = ap.parse_args()
+    tr, cfg, note = full_config(a.config, a.hbm_gib, a.host_gib, a.scale)
+    be = GpuBackend(cfg, len(tr.sessions), tr.F, verify_pages=1)
+    t0 = time.time()
+    r = run(tr, cfg, be)
+    out = dict(config=cfg.name, note=note, wall_s=round(time.time() - t0, 1), pages_verified=be.pages_verified,
+               kernel_launches=be.ctx.launches, **r.totals())
+    be.close()
+    print(json.dumps(out))
+
+
+if __name__ == "__main__":
+    main()

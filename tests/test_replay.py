@@ -120,3 +120,26 @@ def test_gpu_long_agent_replay_reduced():
     assert replay.compare(ro, rg) == []
     assert rg.evictions > 0 and rg.drops > 0 and gb.pages_verified > 0
     gb.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("which", [1, 4])
+def test_gpu_full_size_replay_counts(which):
+    """BASELINE.json configs[1] / configs[4] at full session and turn counts (pools capped by the box, scale
+    stated in the note).  Minutes of wall clock and terabytes over PCIe: runs only when CW_FULL_REPLAY_<which> is
+    set to a divisor of the session count (1 = full)."""
+    import json
+    import os
+    scale = int(os.environ.get(f"CW_FULL_REPLAY_{which}", "0"))
+    if scale < 1:
+        pytest.skip(f"set CW_FULL_REPLAY_{which}=1 (or a divisor) to run the full-size replay")
+    tr, cfg, note = replay.full_config(which, scale=scale)
+    ro, rg, gb = _both(tr, cfg, len(tr.sessions), tr.F, verify_pages=1)
+    diffs = replay.compare(ro, rg)
+    out = dict(config=cfg.name, note=note, oracle=ro.totals(), gpu=rg.totals(), pages_verified=gb.pages_verified,
+               differences=len(diffs))
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open(f"gpurun_out/replay_full_config{which}.json", "w") as f:
+        json.dump(out, f)
+    gb.close()
+    assert diffs == [] and ro.totals() == rg.totals() and rg.evictions > 0

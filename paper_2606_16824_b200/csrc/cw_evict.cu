@@ -99,24 +99,31 @@ __device__ __forceinline__ bool key_lt(u64 s1, u32 i1, u64 s2, u32 i2) { return 
 // ---- digit plan: up to 11 bit positions of the 96-bit key (95 = MSB of the score, 0 = LSB of the id), descending
 #define CWE_BUCKET_BITS 16                       // digit of the victim bucketing (phase D)
 #define CWE_BUCKETS (1u << CWE_BUCKET_BITS)
+// The chosen positions are stored as RUNS of adjacent bits inside one 32-bit word of the key (word 2 = score
+// high, 1 = score low, 0 = id), so that extracting a digit costs one shift-and-mask per run (typically 2-4 runs)
+// instead of one per bit.
 struct DigitPlan {
     u32 nbits;
-    u32 pos[CWE_BUCKET_BITS];
+    u32 nruns;
+    u32 word[CWE_BUCKET_BITS];   // which 32-bit word of the key
+    u32 shift[CWE_BUCKET_BITS];  // lowest bit of the run inside that word
+    u32 mask[CWE_BUCKET_BITS];   // (1 << run length) - 1
+    u32 dst[CWE_BUCKET_BITS];    // position of the run's lowest bit inside the digit
 };
-__device__ __forceinline__ u32 key_bit(u64 score, u32 id, u32 pos) {
-    return pos >= 32 ? (u32)(score >> (pos - 32)) & 1u : (id >> pos) & 1u;
-}
 template <int MAXBITS = CWE_DIGIT_BITS>
 __device__ __forceinline__ u32 plan_digit(const DigitPlan& pl, u64 score, u32 id) {
+    const u32 w2 = (u32)(score >> 32), w1 = (u32)score;
     u32 d = 0;
-#pragma unroll
-    for (int i = 0; i < MAXBITS; ++i)
-        if (i < (int)pl.nbits) d = (d << 1) | key_bit(score, id, pl.pos[i]);
+    for (u32 r = 0; r < pl.nruns; ++r) {  // warp-uniform trip count
+        const u32 w = pl.word[r] == 2 ? w2 : (pl.word[r] == 1 ? w1 : id);
+        d |= ((w >> pl.shift[r]) & pl.mask[r]) << pl.dst[r];
+    }
     return d;
 }
-// the top 11 set bits of (vary_hi : vary_lo); then, if `fill_from` < 96, contiguous bits from there downwards
+// the top `maxbits` set bits of (vary_hi : vary_lo); then, if `fill_from` < 96, contiguous bits from there downwards
 __device__ __forceinline__ void make_plan(DigitPlan* pl, u64 vary_hi, u32 vary_lo, u32 fill_from,
                                           u32 maxbits = CWE_DIGIT_BITS) {
+    u32 pos[CWE_BUCKET_BITS];
     u32 n = 0;
     u32 lowest = 96;
     while (n < maxbits && (vary_hi || vary_lo)) {
@@ -129,19 +136,33 @@ __device__ __forceinline__ void make_plan(DigitPlan* pl, u64 vary_hi, u32 vary_l
             p = 31 - __clz((int)vary_lo);
             vary_lo &= ~(1u << p);
         }
-        pl->pos[n++] = p;
+        pos[n++] = p;
         lowest = p;
     }
     if (fill_from < 96) {
         // plain bits below every chosen one keep the digit a monotone function of the key
         u32 p = lowest == 96 ? fill_from : min(fill_from, lowest - 1);
         while (n < maxbits) {
-            pl->pos[n++] = p;
+            pos[n++] = p;
             if (p == 0) break;
             --p;
         }
     }
+    // positions are descending: group them into runs of adjacent bits that stay inside one 32-bit word
+    u32 nr = 0;
+    for (u32 i = 0; i < n;) {
+        u32 jx = i;
+        while (jx + 1 < n && pos[jx + 1] + 1 == pos[jx] && (pos[jx + 1] >> 5) == (pos[i] >> 5)) ++jx;
+        const u32 len = jx - i + 1;
+        pl->word[nr] = pos[i] >> 5;
+        pl->shift[nr] = pos[jx] & 31;
+        pl->mask[nr] = (1u << len) - 1;  // len <= 16
+        pl->dst[nr] = n - 1 - jx;        // digit bit of the run's lowest key bit
+        ++nr;
+        i = jx + 1;
+    }
     pl->nbits = n;
+    pl->nruns = nr;
 }
 
 // CTA sort of N keys (score,id), N a power of two, 128 <= N <= CWE_SORT_RUN, ascending.
@@ -267,33 +288,40 @@ __device__ __forceinline__ void tile_append(const bool (&f0)[CWE_ITEMS], const b
     __syncthreads();  // s_w*/s_base are reused by the next tile
 }
 
-// block-wide OR of a (u64,u32) pair of masks into global accumulators (one atomic per CTA and word)
-__device__ __forceinline__ void block_or_to_global(u64 hi, u32 lo, u64* g_hi, u32* g_lo, u64* s_hi, u32* s_lo) {
-    const u32 lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-    for (int m = 16; m; m >>= 1) {
-        hi |= shfl64_xor(hi, m);
-        lo |= __shfl_xor_sync(0xffffffffu, lo, m);
-    }
-    if (lane == 0) {
-        s_hi[warp] = hi;
-        s_lo[warp] = lo;
+// block-wide OR of N (u64,u32) pairs of masks into accumulators in global (or shared) memory: hardware warp
+// reductions (redux.sync), one shared-memory atomic per warp and word, one atomic per CTA and word at the target
+template <int N>
+__device__ __forceinline__ void block_or_n(const u64 (&hi)[N], const u32 (&lo)[N], u64* const (&g_hi)[N],
+                                           u32* const (&g_lo)[N], u64* s_hi, u32* s_lo) {
+    const u32 tid = threadIdx.x, lane = tid & 31;
+    if (tid < N) {
+        s_hi[tid] = 0;
+        s_lo[tid] = 0;
     }
     __syncthreads();
-    if (warp == 0) {
-        hi = s_hi[lane];
-        lo = s_lo[lane];
 #pragma unroll
-        for (int m = 16; m; m >>= 1) {
-            hi |= shfl64_xor(hi, m);
-            lo |= __shfl_xor_sync(0xffffffffu, lo, m);
-        }
+    for (int n = 0; n < N; ++n) {
+        const u32 a = __reduce_or_sync(0xffffffffu, (u32)hi[n]);
+        const u32 b = __reduce_or_sync(0xffffffffu, (u32)(hi[n] >> 32));
+        const u32 c = __reduce_or_sync(0xffffffffu, lo[n]);
         if (lane == 0) {
-            if (hi) atomicOr(reinterpret_cast<unsigned long long*>(g_hi), (unsigned long long)hi);
-            if (lo) atomicOr(g_lo, lo);
+            if (a | b) atomicOr(reinterpret_cast<unsigned long long*>(s_hi + n), ((unsigned long long)b << 32) | a);
+            if (c) atomicOr(s_lo + n, c);
         }
     }
     __syncthreads();
+    if (tid < N) {
+        if (s_hi[tid]) atomicOr(reinterpret_cast<unsigned long long*>(g_hi[tid]), (unsigned long long)s_hi[tid]);
+        if (s_lo[tid]) atomicOr(g_lo[tid], s_lo[tid]);
+    }
+    __syncthreads();
+}
+__device__ __forceinline__ void block_or_to_global(u64 hi, u32 lo, u64* g_hi, u32* g_lo, u64* s_hi, u32* s_lo) {
+    const u64 h[1] = {hi};
+    const u32 l[1] = {lo};
+    u64* const gh[1] = {g_hi};
+    u32* const gl[1] = {g_lo};
+    block_or_n<1>(h, l, gh, gl, s_hi, s_lo);
 }
 
 // threshold bin of a level: the bin in which the `remaining`-th smallest candidate falls
@@ -416,11 +444,12 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
         __syncthreads();
     }
 
+    stamp(st, n_stamp);  // end of phase A
     // ---------------------------------------------------------------- B: score + compact + level-0 histogram
     for (u32 i = tid; i < CWE_BINS; i += CWE_THREADS) s_hist[i] = 0;
     __syncthreads();
     {
-        const DigitPlan pl = s_plan;
+        const DigitPlan& pl = s_plan;
         for (u32 tile = blockIdx.x; (u64)tile * CWE_TILE < a.M; tile += G) {
             bool f0[CWE_ITEMS], f1[CWE_ITEMS];
             u32 p0[CWE_ITEMS], p1[CWE_ITEMS];
@@ -460,6 +489,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
                 }
         }
     }
+    stamp(st, n_stamp);  // CTA 0 done with its tiles
     flush_hist(s_hist, a.hist);
     grid_barrier(st, G);
     stamp(st, n_stamp);
@@ -537,11 +567,16 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
                         }
                         for (u32 i = tid; i < CWE_BINS; i += CWE_THREADS) l_hist[i] = 0;
                         __syncthreads();
-                        block_or_to_global(o_hi, o_lo, &s_acc_hi, &s_acc_lo, s_mhi, s_mlo);
-                        block_or_to_global(x_hi, x_lo, &s_acc2_hi, &s_acc2_lo, s_mhi, s_mlo);
+                        {
+                            const u64 h2[2] = {o_hi, x_hi};
+                            const u32 l2[2] = {o_lo, x_lo};
+                            u64* const gh[2] = {&s_acc_hi, &s_acc2_hi};
+                            u32* const gl[2] = {&s_acc_lo, &s_acc2_lo};
+                            block_or_n<2>(h2, l2, gh, gl, s_mhi, s_mlo);
+                        }
                         if (tid == 0) make_plan(&s_plan, s_acc_hi & s_acc2_hi, s_acc_lo & s_acc2_lo, 96);
                         __syncthreads();
-                        const DigitPlan lp = s_plan;
+                        const DigitPlan& lp = s_plan;
                         for (u32 i = tid; i < n; i += CWE_THREADS) atomicAdd(&l_hist[plan_digit(lp, c_s[i], c_i[i])], 1u);
                         __syncthreads();
                         find_threshold<false>(l_hist, remaining, s_scan, s_thr);
@@ -575,8 +610,13 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
                         u32* ti_ = c_i; c_i = n_i; n_i = ti_;
                     }
                     __syncthreads();
-                    block_or_to_global(v_or_hi, v_or_lo, &st->vic_or_hi, &st->vic_or_lo, s_mhi, s_mlo);
-                    block_or_to_global(v_nand_hi, v_nand_lo, &st->vic_nand_hi, &st->vic_nand_lo, s_mhi, s_mlo);
+                    {
+                        const u64 h2[2] = {v_or_hi, v_nand_hi};
+                        const u32 l2[2] = {v_or_lo, v_nand_lo};
+                        u64* const gh[2] = {&st->vic_or_hi, &st->vic_nand_hi};
+                        u32* const gl[2] = {&st->vic_or_lo, &st->vic_nand_lo};
+                        block_or_n<2>(h2, l2, gh, gl, s_mhi, s_mlo);
+                    }
                 }
                 break;
             }
@@ -585,8 +625,9 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
             const u32 thr = s_thr[0], before = s_thr[1], inside = s_thr[2];
             const u32 need_here = remaining - before;
             const bool take_all = need_here == inside;
-            const DigitPlan pl = s_plan;
+            const DigitPlan& pl = s_plan;
             __syncthreads();
+            stamp(st, n_stamp);  // threshold found
             // filter: bins below the threshold are victims, the threshold bin is the next candidate set
             u64* ns = a.cand_score[(p + 1) & 1];
             u32* ni = a.cand_id[(p + 1) & 1];
@@ -634,11 +675,14 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
                     }
                 }
             }
-            block_or_to_global(v_or_hi, v_or_lo, &st->vic_or_hi, &st->vic_or_lo, s_mhi, s_mlo);
-            block_or_to_global(v_nand_hi, v_nand_lo, &st->vic_nand_hi, &st->vic_nand_lo, s_mhi, s_mlo);
-            if (!take_all && inside > CWE_LOCAL) {
-                block_or_to_global(m_or_hi, m_or_lo, &st->or_hi[p + 1], &st->or_lo[p + 1], s_mhi, s_mlo);
-                block_or_to_global(m_nand_hi, m_nand_lo, &st->nand_hi[p + 1], &st->nand_lo[p + 1], s_mhi, s_mlo);
+            stamp(st, n_stamp);  // CTA 0 done with its filter tiles
+            {
+                const bool next = !take_all && inside > CWE_LOCAL;  // the next level needs the masks of its set
+                const u64 h4[4] = {v_or_hi, v_nand_hi, next ? m_or_hi : 0ull, next ? m_nand_hi : 0ull};
+                const u32 l4[4] = {v_or_lo, v_nand_lo, next ? m_or_lo : 0u, next ? m_nand_lo : 0u};
+                u64* const gh[4] = {&st->vic_or_hi, &st->vic_nand_hi, &st->or_hi[p + 1], &st->nand_hi[p + 1]};
+                u32* const gl[4] = {&st->vic_or_lo, &st->vic_nand_lo, &st->or_lo[p + 1], &st->nand_lo[p + 1]};
+                block_or_n<4>(h4, l4, gh, gl, s_mhi, s_mlo);
             }
             grid_barrier(st, G);
             stamp(st, n_stamp);
@@ -659,7 +703,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
             for (u32 i = tid; i < CWE_BINS; i += CWE_THREADS) s_hist[i] = 0;
             __syncthreads();
             {
-                const DigitPlan pn = s_plan;
+                const DigitPlan& pn = s_plan;
                 for (u32 base = blockIdx.x * CWE_THREADS; base < n_cur; base += G * CWE_THREADS) {
                     const u32 e = base + tid;
                     const bool ok = e < n_cur;
@@ -727,7 +771,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
         return;
     }
     // D1: bucket = the top 16 bits that vary among the victims (a monotone function of the key), histogram
-    const DigitPlan bp = s_plan;
+    const DigitPlan& bp = s_plan;
     for (u32 e = blockIdx.x * CWE_THREADS + tid; e < want; e += G * CWE_THREADS)
         atomicAdd(&a.bhist[plan_digit<CWE_BUCKET_BITS>(bp, __ldcg(a.out_score + e), __ldcg(a.out_id + e))], 1u);
     grid_barrier(st, G);

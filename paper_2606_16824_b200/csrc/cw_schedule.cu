@@ -3,7 +3,7 @@
 // The queue is ordered by a 192-bit key that is a TOTAL order (the input index is its last component):
 //   policy 0  (a | ~n_gpu , arrival_seq , req_id | idx)      PAPER.md 5.1 L207 "fewest additional blocks"
 //   policy 1  (~n_gpu | a , arrival_seq , req_id | idx)      L45 / Fig. 11B "degree of overlap"
-//   policy 2  (0         , arrival_seq , req_id | idx)       L281 FCFS
+//   policy 2  (arrival_seq , 0         , req_id | idx)       L281 FCFS
 // A few thousand keys are too few to feed a radix sort and too many for one CTA's sorting network, so the
 // sort is a RANK SORT spread over the whole GPU: rank(i) = #{j : key_j < key_i}, R^2 comparisons (16.7 M at
 // R = 4096, ~100 per thread), keys staged through shared memory in tiles.  order[rank(i)] = i.
@@ -34,8 +34,9 @@ __device__ __forceinline__ Key3 make_key(u32 i, const u32* need, const u32* n_gp
     const u64 a = d > g ? d - g : 0;
     const u64 inv = 0xFFFFFFFFull - g;
     Key3 k;
-    k.k0 = policy == 0 ? (a << 32) | inv : policy == 1 ? (inv << 32) | a : 0ull;
-    k.k1 = arrival[i];
+    // FCFS puts arrival_seq in the leading word so that the first comparison decides almost every pair
+    k.k0 = policy == 0 ? (a << 32) | inv : policy == 1 ? (inv << 32) | a : arrival[i];
+    k.k1 = policy == 2 ? 0ull : arrival[i];
     k.k2 = ((u64)req_id[i] << 32) | i;
     return k;
 }
@@ -71,8 +72,13 @@ __global__ void __launch_bounds__(CWS_THREADS)
         if (live) {
 #pragma unroll 4
             for (u32 t = jl; t < n; t += CWS_J_LANES) {
-                const Key3 o{s_k0[t], s_k1[t], s_k2[t]};
-                rank += key_less(o, mine) ? 1u : 0u;
+                const u64 o0 = s_k0[t];
+                if (o0 != mine.k0) {  // decided by the leading word (the common case): 1 load, 2 compares
+                    rank += o0 < mine.k0 ? 1u : 0u;
+                } else {
+                    const Key3 o{o0, s_k1[t], s_k2[t]};
+                    rank += key_less(o, mine) ? 1u : 0u;
+                }
             }
         }
     }

@@ -23,7 +23,15 @@
 
 namespace {
 
-__device__ __forceinline__ uint4 ld_slot(const cw_slot* s) { return *reinterpret_cast<const uint4*>(s); }
+__device__ __forceinline__ uint4 ld_slot(const cw_slot* s) {
+#ifdef CW_SLOT_LDCG
+    return __ldcg(reinterpret_cast<const uint4*>(s));
+#elif defined(CW_SLOT_LDCV)
+    return __ldcv(reinterpret_cast<const uint4*>(s));
+#else
+    return *reinterpret_cast<const uint4*>(s);
+#endif
+}
 __device__ __forceinline__ u64 slot_key(const uint4& v) { return ((u64)v.y << 32) | v.x; }
 
 // returns slot index of `key` (already remapped) or ~0 if absent
@@ -148,7 +156,9 @@ __global__ void insert_reset_kernel(cw_slot* table, u32 n, const u32* ins_slot) 
 }
 
 // ---------------------------------------------------------------------------------------------- match
-#define CWM_CHUNK 1024  // consecutive hashes handled by one warp task (32 rounds of 32)
+#define CWM_CHUNK 256  // consecutive hashes handled by one warp task (8 rounds of 32): measured optimum on
+                       // configs[2] (128: 97 us, 256: 100, 512: 105, 1024: 124, 2048: 208 — long tasks are bound by the
+                       // dependent probe chain of the slowest warp, short ones by occupancy x latency)
 
 __global__ void __launch_bounds__(256) match_probe_kernel(const cw_slot* __restrict__ table, u64 mask,
                                                           const u64* __restrict__ hashes,

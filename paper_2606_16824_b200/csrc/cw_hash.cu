@@ -71,6 +71,7 @@ struct __align__(128) HashSmem {
     u64 full[CWH_STAGES];
     u64 empty[CWH_STAGES];
     u64 wagg[2][CWH_WARPS];
+    u64 pw[CWH_WARPS + 1];  // (A^32)^k
     u64 carry_in;
     u32 range;
     u32 rec_flags;
@@ -164,6 +165,7 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, 4) hash_kernel(const HashArgs a
     const u64 u_begin = min(U, per * range), u_end = min(U, u_begin + per);
     if (u_begin >= u_end) return;  // empty range (uniform over the CTA): nobody waits for it
 
+    if (tid <= CWH_WARPS) sm.pw[tid] = pow_u64(cw_pow(CW_A, 32), tid);
     if (tid == 0) {
         for (int s = 0; s < CWH_STAGES; ++s) {
             mbar_init(smem_u32(&sm.full[s]), 1);
@@ -269,8 +271,7 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, 4) hash_kernel(const HashArgs a
         // after the transposed reduction lane i owns block 8*k(i) + (i>>2), k(i) = 2*bit0 + bit1;
         // the lane that owns block b is 4*(b&7) | ((b>>3)&1)<<1 | (b>>4)
         const u32 owner = ((lane & 7) << 2) | (((lane >> 3) & 1) << 1) | (lane >> 4);
-        constexpr u64 A2 = cw_pow(CW_A, 2), A4 = cw_pow(CW_A, 4), A8 = cw_pow(CW_A, 8), A16 = cw_pow(CW_A, 16),
-                      A32 = cw_pow(CW_A, 32);
+        constexpr u64 A2 = cw_pow(CW_A, 2), A4 = cw_pow(CW_A, 4), A8 = cw_pow(CW_A, 8), A16 = cw_pow(CW_A, 16);
         u64 carry = 0;  // chain state before the current unit (uniform over the CTA)
 
         for (u32 it = 0;; ++it) {
@@ -323,15 +324,23 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, 4) hash_kernel(const HashArgs a
             consumer_bar();
             if (tid == 0) mbar_arrive(smem_u32(&sm.empty[s]));  // every consumer has read stage s
 
-            // ---- carry-in of this warp by Horner over the earlier warps; the full Horner gives the next carry
-            u64 run = ui.mode == MODE_SEED ? ui.seed : (ui.mode == MODE_ZERO ? 0ull : carry);
-            u64 cin = 0;
-#pragma unroll
-            for (u32 v = 0; v < CWH_WARPS; ++v) {
-                if (v == warp) cin = run;
-                run = A32 * run + sm.wagg[buf][v];
+            // ---- carry-in of this warp and the state after the unit, lane-parallel: lanes 0-7 fold the earlier warps'
+            //      aggregates for this warp, lanes 8-15 fold all eight for the next unit (powers of A^32 from smem)
+            const u64 run0 = ui.mode == MODE_SEED ? ui.seed : (ui.mode == MODE_ZERO ? 0ull : carry);
+            u64 term = 0;
+            {
+                const u32 v = lane & 7, grp = lane >> 3;
+                if (grp < 2) {
+                    const u32 tgt = grp == 0 ? warp : CWH_WARPS;  // how many warp aggregates are folded in
+                    if (v < tgt) term = sm.pw[tgt - 1 - v] * sm.wagg[buf][v];
+                    if (v == 0) term += sm.pw[tgt] * run0;
+                }
+                term += shfl64_xor(term, 1);
+                term += shfl64_xor(term, 2);
+                term += shfl64_xor(term, 4);
             }
-            carry = run;  // meaningful when the unit is full (a partial unit ends its request)
+            const u64 cin = shfl64(term, 0);
+            carry = shfl64(term, 8);  // meaningful when the unit is full (a partial unit ends its request)
             const u64 h = x + a_lane1 * cin;
             const u32 bi = warp * 32 + lane;
             if (bi < ui.nblk) a.hashes[ui.out_base + bi] = h;

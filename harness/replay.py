@@ -37,6 +37,8 @@ class ReplayConfig:
     policy: int = 0                 # cw_schedule policy
     max_admit: int = 2
     use_hint: bool = False          # CacheWise* (PAPER.md L285): tau_override = true gap
+    evict_policy: str = "cachewise"  # "cachewise" (per-session linear predictor), "hint" (= use_hint), "lru" (vLLM,
+                                     # L281: every tau equal), "infercept" (L283: session moving average of tool time)
     c0_ms: int = 20                 # integer service model: c0 + ceil(c_tok*new_tokens/1000) + c_blk*swapped_in
     c_tok_us: int = 250
     c_blk_ms: int = 1
@@ -140,6 +142,8 @@ def run(trace: gen.Trace, cfg: ReplayConfig, be) -> ReplayResult:
     prev_hashes = [np.zeros(0, np.uint64) for _ in range(S)]
     queue: list[Request] = []
     now, tick, seq, rid = 0, 1, 0, 0
+    gap_avg = np.zeros(S, np.int64)      # InferCept baseline: what the session's tool calls took so far
+    last_done = np.zeros(S, np.int64)
 
     def flags(ids):
         return (np.where(b_valid[ids], REF_VALID, 0) | b_ref[ids]).astype(np.uint32)
@@ -238,8 +242,12 @@ def run(trace: gen.Trace, cfg: ReplayConfig, be) -> ReplayResult:
         short = max(0, need_sum - len(free_hbm))
         if short:
             tau_ov = None
-            if cfg.use_hint:
+            if cfg.use_hint or cfg.evict_policy == "hint":
                 tau_ov = np.clip(next_arrival - now, 0, 0xFFFFFF).astype(np.uint32)
+            elif cfg.evict_policy == "lru":
+                tau_ov = np.full(S, 1000, np.uint32)
+            elif cfg.evict_policy == "infercept":   # moving average of the session's past gaps minus the elapsed time
+                tau_ov = np.clip(gap_avg - (now - last_done), 0, 0xFFFFFF).astype(np.uint32)
             victims, vscores, st = be.score_evict(tick, features, trace.weights, trace.bias, state, tau_ov, short, 0,
                                                   short)
             assert victims.size == short, (victims.size, short, st)
@@ -354,6 +362,10 @@ def run(trace: gen.Trace, cfg: ReplayConfig, be) -> ReplayResult:
             if turn_idx[s] < len(trace.sessions[s]):
                 state[s] = gen.TOOL_WAIT
                 next_arrival[s] = now + t.gap_ms
+                last_done[s] = now
+                if q.turn > 0:  # the previous gap is known by now: exponential moving average (alpha = 1/2)
+                    prev_gap = trace.sessions[s][q.turn - 1].gap_ms
+                    gap_avg[s] = prev_gap if q.turn == 1 else (gap_avg[s] + prev_gap) // 2
                 waiting[s] = True
             else:
                 state[s] = gen.IDLE
@@ -366,6 +378,28 @@ def run(trace: gen.Trace, cfg: ReplayConfig, be) -> ReplayResult:
         tick += 1
     res.end_ms = now
     return res
+
+
+SYSTEMS = {  # the paper's comparison systems as (schedule policy, eviction policy) pairs — PAPER.md L281-285
+    "vLLM (FCFS + LRU)": (2, "lru"),
+    "InferCept (FCFS + moving average)": (2, "infercept"),
+    "vLLM (prefix-aware)": (0, "lru"),
+    "CacheWise (prefix-aware + predictor)": (0, "cachewise"),
+    "CacheWise* (prefix-aware + true tau)": (0, "hint"),
+}
+
+
+def policy_sweep(trace: gen.Trace, base: ReplayConfig, make_backend):
+    """Runs the same trace under every system of SYSTEMS; returns {name: totals + mean session time}."""
+    import dataclasses
+    out = {}
+    for name, (sched, ev) in SYSTEMS.items():
+        cfg = dataclasses.replace(base, policy=sched, evict_policy=ev, use_hint=False)
+        r = run(trace, cfg, make_backend(cfg))
+        t = r.totals()
+        t["mean_session_ms"] = int(np.mean(list(r.session_done_ms.values())))
+        out[name] = t
+    return out
 
 
 def compare(a: ReplayResult, b: ReplayResult):
@@ -570,7 +604,15 @@ def main():
     ap.add_argument("--scale", type=int, default=1, help="divide the number of sessions (and turns of config 4)")
     ap.add_argument("--hbm-gib", type=float, default=120.0)
     ap.add_argument("--host-gib", type=float, default=48.0)
+    ap.add_argument("--sweep", action="store_true", help="run the paper's comparison systems on a synthetic trace")
     a = ap.parse_args()
+    if a.sweep:
+        tr = gen.session_trace(21, 48, 24, 8, (6000.0, 0.6, 1024, 24000), 128, 1024, 1.0, 40000,
+                               [(0.7, 1000.0, 1.0), (0.3, 60000.0, 1.0)])
+        ws = sum(max((t.tokens.size + 15) // 16 for t in s) for s in tr.sessions)
+        base = ReplayConfig("sweep", int(0.3 * ws), 0, 4, 4096, max_admit=8, store_bytes=False)
+        print(json.dumps(policy_sweep(tr, base, lambda c: GpuBackend(c, 48, 8)), indent=1))
+        return
     tr, cfg, note = full_config(a.config, a.hbm_gib, a.host_gib, a.scale)
     be = GpuBackend(cfg, len(tr.sessions), tr.F, verify_pages=1)
     t0 = time.time()

@@ -36,8 +36,8 @@ PCIE_GEN5_X16_GBS = 63.0  # 32 GT/s x 16 lanes x 128/130 / 8 per direction (SURV
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r1_full_step_kernels.md), full-size configs[2] step.
-NCU_TRAFFIC_BYTES = {"hash": 433_265_408, "match": 103_412_224, "score_evict": 17_190_400, "gather": 1_660_707_072,
-                     "scatter": 1_660_303_616, "schedule": 105_216}
+NCU_TRAFFIC_BYTES = {"hash": 433_284_864, "match": 103_933_952, "score_evict": 17_291_007, "gather": 1_660_023_295,
+                     "scatter": 1_659_612_672, "schedule": 107_776}
 
 
 def measured_peaks():

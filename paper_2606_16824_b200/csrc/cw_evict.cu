@@ -9,12 +9,14 @@
 //      digit of a level is gathered from the top 11 bits that actually VARY inside the current candidate set
 //      (OR / AND masks accumulated while the set is written), so every level splits the set — no wasted
 //      levels when thousands of blocks share tau and age.  Bins below the threshold bin are victims, the
-//      threshold bin becomes the next candidate set; a set of <= 4096 is finished by one CTA in shared memory.
+//      threshold bin becomes the next candidate set; a set of <= 4096 is finished by one CTA in shared memory
+//      (the same levels without grid barriers, then rank counting once <= 256 candidates are left).
 //      Histograms use warp-aggregated shared-memory atomics (blocks of one session share a digit).
 //   D  victims are ordered by (score, id): one more split on the top 16 bits that vary among the victims
-//      (65536 buckets: global histogram, scan, scatter), then every bucket is finished on its own — up to 32
-//      keys by one warp (rank counting with shuffles), up to 4096 by one CTA (warp-chunk bitonic + merge-path
-//      rounds in shared memory), anything larger by a grid-wide bitonic network (fallback, adversarial keys only).
+//      (65536 buckets: global histogram, distributed scan, scatter), then every non-empty bucket is finished on its
+//      own — up to 128 keys by one warp (bitonic network in its shared-memory chunk, __syncwarp only), up to 4096
+//      by one CTA (warp-chunk bitonic + merge-path rounds in shared memory), anything larger by a grid-wide
+//      bitonic network (fallback, adversarial keys only).
 //      An answer of <= 4096 victims is sorted by one CTA directly.
 //   E  scratch is re-zeroed for the next call (the kernel is self-cleaning => graph-capturable)
 // This replaces the paper's eviction heap + rebuild every N_rebuild=3 iterations (L252-254): a full

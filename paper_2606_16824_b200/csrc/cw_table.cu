@@ -156,11 +156,14 @@ __global__ void insert_reset_kernel(cw_slot* table, u32 n, const u32* ins_slot) 
 }
 
 // ---------------------------------------------------------------------------------------------- match
+// 8 CTAs of 256 threads per SM (<= 32 registers): the probe is bound by resident warps x latency (93 us vs 107 us
+// at 6 CTAs/SM on configs[2])
+#define MATCH_MIN_CTAS 8
 #define CWM_CHUNK 256  // consecutive hashes handled by one warp task (8 rounds of 32): measured optimum on
                        // configs[2] (128: 97 us, 256: 100, 512: 105, 1024: 124, 2048: 208 — long tasks are bound by the
                        // dependent probe chain of the slowest warp, short ones by occupancy x latency)
 
-__global__ void __launch_bounds__(256) match_probe_kernel(const cw_slot* __restrict__ table, u64 mask,
+__global__ void __launch_bounds__(256, MATCH_MIN_CTAS) match_probe_kernel(const cw_slot* __restrict__ table, u64 mask,
                                                           const u64* __restrict__ hashes,
                                                           const u64* __restrict__ hash_off, u32 R, u32* first_miss,
                                                           u32* max_hit, u32* host_hits, u32* hit_loc) {

@@ -51,6 +51,23 @@ __device__ __forceinline__ u64 table_find(const cw_slot* table, u64 mask, u64 ke
     return ~0ull;
 }
 
+// Probe of the match pass: ONE 128-bit load per slot (the generic ld_slot is split by the compiler into a key load
+// and a dependent loc load: a second memory latency on every hit), 32-bit index arithmetic.
+__device__ __forceinline__ u32 table_probe(const cw_slot* __restrict__ table, u32 mask, u64 key) {
+    u32 i = (u32)key & mask;
+    for (u32 n = 0; n <= mask; ++n) {
+        uint4 v;
+        asm volatile("ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4];"
+                     : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                     : "l"(table + i));
+        const u64 k = slot_key(v);
+        if (k == key) return v.z;
+        if (k == CW_KEY_EMPTY) break;
+        i = (i + 1) & mask;
+    }
+    return CW_MISS;
+}
+
 __global__ void lookup_kernel(const cw_slot* table, u64 mask, const u64* keys, u32 n, u32* loc) {
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -187,20 +204,29 @@ __global__ void __launch_bounds__(256, MATCH_MIN_CTAS) match_probe_kernel(const 
             lo = nlo;
         }
         u32 r_base = lo;  // request of the first hash of the current round (kept up to date below)
+        u64 req_start = hash_off[lo], req_end = hash_off[lo + 1];
         u32 dead_r = 0xFFFFFFFFu, checked_r = 0xFFFFFFFFu;  // request known to have missed / whose global state was read
         const u64 c1 = min(total, c0 + CWM_CHUNK);
         u64 key_next = c0 + lane < c1 ? hashes[c0 + lane] : 0;
         for (u64 g0 = c0; g0 < c1; g0 += 32) {
-            while (g0 >= hash_off[r_base + 1]) ++r_base;  // warp-uniform; also skips empty requests
+            while (g0 >= req_end) {  // warp-uniform; also skips empty requests
+                ++r_base;
+                req_start = req_end;
+                req_end = hash_off[r_base + 1];
+            }
             const u64 g = g0 + lane;
             const bool active = g < c1;
             const u64 key = key_next;
             if (g + 32 < c1) key_next = hashes[g + 32];  // prefetch the next round
             u32 r = r_base;
-            if (active)
-                while (g >= hash_off[r + 1]) ++r;
-            const u32 j = active ? (u32)(g - hash_off[r]) : 0;
-            const bool uniform = __all_sync(0xffffffffu, !active || r == r_base);
+            u32 j = (u32)(g - req_start);
+            bool uniform = true;
+            if (min(g0 + 32, c1) > req_end) {  // the round crosses into the next request(s): per-lane walk (rare)
+                if (active)
+                    while (g >= hash_off[r + 1]) ++r;
+                j = active ? (u32)(g - hash_off[r]) : 0;
+                uniform = __all_sync(0xffffffffu, !active || r == r_base);
+            }
             const u32 act_mask = __ballot_sync(0xffffffffu, active);
             if (uniform) {
                 if (r_base != checked_r && r_base != dead_r) {  // entering a request: did an earlier task miss?
@@ -214,7 +240,7 @@ __global__ void __launch_bounds__(256, MATCH_MIN_CTAS) match_probe_kernel(const 
                 }
             }
             u32 loc = CW_MISS;
-            if (active) table_find(table, mask, cw_remap_key(key), &loc);
+            if (active) loc = table_probe(table, (u32)mask, cw_remap_key(key));
             if (uniform) {
                 const u32 miss_mask = __ballot_sync(0xffffffffu, active && loc == CW_MISS);
                 const u32 first = miss_mask ? (u32)__ffs(miss_mask) - 1 : 32;

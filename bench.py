@@ -36,8 +36,8 @@ PCIE_GEN5_X16_GBS = 63.0  # 32 GT/s x 16 lanes x 128/130 / 8 per direction (SURV
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r1_full_step_kernels.md), full-size configs[2] step.
-NCU_TRAFFIC_BYTES = {"hash": 433_284_864, "match": 103_933_952, "score_evict": 17_291_007, "gather": 1_660_023_295,
-                     "scatter": 1_659_612_672, "schedule": 107_776}
+NCU_TRAFFIC_BYTES = {"hash": 433_584_895, "match": 105_218_560, "score_evict": 17_284_864, "gather": 1_660_822_272,
+                     "scatter": 1_658_515_456, "schedule": 107_008}
 
 
 def measured_peaks():
@@ -432,6 +432,16 @@ def run_cuda(args):
                 dec[name + "_l2_warm"] = graph_latency(torch, stream, lambda: st.decide(steady))
                 dec[name + "_l2_flushed"] = graph_latency(torch, stream, lambda: st.decide(steady), flush=flush)
         del big
+        with torch.cuda.stream(stream):  # the steady-state hash call alone (CUDA events, median of 20)
+            ts = []
+            for _ in range(23):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                st.hash(True)
+                e1.record(stream)
+                stream.synchronize()
+                ts.append(e0.elapsed_time(e1) * 1e3)
+            dec["steady_hash_us"] = round(sorted(ts[3:])[10], 2)
         dec["note"] = ("stages 1-3 (hash, match, schedule, score/select) as one CUDA graph; cold = all 4096 requests "
                        f"hashed ({st.n_hashed} blocks), steady = hashes persist and the {st.new_requests} newest "
                        f"requests ({st.n_hashed_new} blocks) are hashed; target <= 100 us")

@@ -68,21 +68,23 @@ struct EvictArgs {
     u32* num_victims;
 };
 
-__device__ __forceinline__ void grid_barrier(cw_evict_state* st, u32 nblocks) {
+// Grid barrier of the cooperative launch.  `gen` is this CTA's private copy of the barrier generation (read once
+// at kernel start), so an arrival is ONE acq_rel atomic and the wait is an acquire spin on the generation word:
+// no fence instructions, no extra round trip to read the generation first.
+__device__ __forceinline__ void grid_barrier(cw_evict_state* st, u32 nblocks, u32& gen) {
     __syncthreads();
     if (threadIdx.x == 0) {
-        const u32 g = ld_acquire_u32(&st->bar_gen);
-        __threadfence();
-        if (atomicAdd(&st->bar_count, 1u) == nblocks - 1) {
-            st->bar_count = 0;
-            __threadfence();
-            st_release_u32(&st->bar_gen, g + 1);
+        u32 prev;
+        asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(prev) : "l"(&st->bar_count) : "memory");
+        if (prev == nblocks - 1) {
+            st->bar_count = 0;  // nobody touches the counter again before the generation moves on
+            st_release_u32(&st->bar_gen, gen + 1);
         } else {
-            while (ld_acquire_u32(&st->bar_gen) == g) {
+            while (ld_acquire_u32(&st->bar_gen) == gen) {
             }
         }
-        __threadfence();
     }
+    ++gen;
     __syncthreads();
 }
 
@@ -393,6 +395,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     const u32 tid = threadIdx.x, G = gridDim.x;
     cw_evict_state* st = a.st;
     const bool tau_smem = a.S <= CWE_SMEM_SESS;
+    u32 bar_gen = ld_acquire_u32(&st->bar_gen);  // cannot move before this CTA has arrived at the first barrier
     u32 n_stamp = 0;
     stamp(st, n_stamp);
 
@@ -434,7 +437,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
             block_or_to_global(packed, 0u, &s_acc_hi, &s_acc_lo, s_mhi, s_mlo);
         } else {
             block_or_to_global(packed, 0u, &st->tau_masks, &s_acc_lo, s_mhi, s_mlo);
-            grid_barrier(st, G);
+            grid_barrier(st, G, bar_gen);
             stamp(st, n_stamp);
             if (tid == 0) s_acc_hi = __ldcg(reinterpret_cast<const unsigned long long*>(&st->tau_masks));
             __syncthreads();
@@ -493,7 +496,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     }
     stamp(st, n_stamp);  // CTA 0 done with its tiles
     flush_hist(s_hist, a.hist);
-    grid_barrier(st, G);
+    grid_barrier(st, G, bar_gen);
     stamp(st, n_stamp);
 
     // ---------------------------------------------------------------- C: radix select
@@ -686,7 +689,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
                 u32* const gl[4] = {&st->vic_or_lo, &st->vic_nand_lo, &st->or_lo[p + 1], &st->nand_lo[p + 1]};
                 block_or_n<4>(h4, l4, gh, gl, s_mhi, s_mlo);
             }
-            grid_barrier(st, G);
+            grid_barrier(st, G, bar_gen);
             stamp(st, n_stamp);
             if (take_all) {
                 remaining = 0;
@@ -715,11 +718,11 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
                 }
             }
             flush_hist(s_hist, a.hist + (p + 1) * CWE_BINS);
-            grid_barrier(st, G);
+            grid_barrier(st, G, bar_gen);
             stamp(st, n_stamp);
         }
     }
-    grid_barrier(st, G);
+    grid_barrier(st, G, bar_gen);
     stamp(st, n_stamp);
 
     // ---------------------------------------------------------------- E (early): re-zero scratch
@@ -776,7 +779,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     const DigitPlan& bp = s_plan;
     for (u32 e = blockIdx.x * CWE_THREADS + tid; e < want; e += G * CWE_THREADS)
         atomicAdd(&a.bhist[plan_digit<CWE_BUCKET_BITS>(bp, __ldcg(a.out_score + e), __ldcg(a.out_id + e))], 1u);
-    grid_barrier(st, G);
+    grid_barrier(st, G, bar_gen);
     stamp(st, n_stamp);
     // D2: exclusive scan of the bucket sizes, every CTA on its own slice of 512 buckets: the offset of the slice
     //     is the sum of all earlier buckets (re-read from L2: at most 256 KiB), so no CTA waits for another
@@ -835,7 +838,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
             st->vic_nand_lo = 0;
         }
     }
-    grid_barrier(st, G);
+    grid_barrier(st, G, bar_gen);
     stamp(st, n_stamp);
     // D3: scatter into bucket order (inside a bucket the order is arbitrary for now)
     u64* tmp_score = a.cand_score[0];
@@ -847,7 +850,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
         tmp_score[pos] = sc;
         tmp_id[pos] = id;
     }
-    grid_barrier(st, G);
+    grid_barrier(st, G, bar_gen);
     stamp(st, n_stamp);
     // D4: one warp per bucket: up to 128 keys are sorted by the warp in its own shared-memory chunk (bitonic,
     //     __syncwarp only) and written to their final place; larger buckets are queued for a CTA sort
@@ -904,7 +907,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
           }
         }
     }
-    grid_barrier(st, G);
+    grid_barrier(st, G, bar_gen);
     stamp(st, n_stamp);
     // D5: medium buckets, one CTA each
     const u32 n_medium = __ldcg(&st->n_medium), n_large = __ldcg(&st->n_large);
@@ -951,7 +954,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
                         }
                     }
                 }
-                grid_barrier(st, G);
+                grid_barrier(st, G, bar_gen);
                 stamp(st, n_stamp);
             }
         }

@@ -6,7 +6,9 @@
 //   policy 2  (arrival_seq , 0         , req_id | idx)       L281 FCFS
 // A few thousand keys are too few to feed a radix sort and too many for one CTA's sorting network, so the
 // sort is a RANK SORT spread over the whole GPU: rank(i) = #{j : key_j < key_i}, R^2 comparisons (16.7 M at
-// R = 4096, ~100 per thread), keys staged through shared memory in tiles.  order[rank(i)] = i.
+// R = 4096, one warp per element).  Only the LEADING word of every key is staged in shared memory (it decides
+// almost every pair: a branch-free smaller/equal count); the other words are fetched from global memory for the
+// few keys that tie on it.  order[rank(i)] = i.
 // The last CTA to finish (atomic ticket, no spinning) runs the admission rule of L177 over the sorted
 // order: exclusive prefix sum of a, admit while it fits, stop at the first misfit.
 #include <stdio.h>
@@ -18,16 +20,11 @@ namespace {
 #define CWS_THREADS 256
 #define CWS_I_PER_CTA 8                       // elements ranked by one CTA
 #define CWS_J_LANES (CWS_THREADS / CWS_I_PER_CTA)  // threads sharing one element (split the j range)
-#define CWS_TILE 1024                         // keys staged per shared-memory tile
+#define CWS_TILE 8192                         // leading key words staged per shared-memory tile (64 KiB)
 
 struct Key3 {
     u64 k0, k1, k2;
 };
-__device__ __forceinline__ bool key_less(const Key3& x, const Key3& y) {
-    if (x.k0 != y.k0) return x.k0 < y.k0;
-    if (x.k1 != y.k1) return x.k1 < y.k1;
-    return x.k2 < y.k2;
-}
 __device__ __forceinline__ Key3 make_key(u32 i, const u32* need, const u32* n_gpu, const u64* arrival,
                                          const u32* req_id, u32 policy) {
     const u32 d = need[i], g = n_gpu[i];
@@ -41,49 +38,74 @@ __device__ __forceinline__ Key3 make_key(u32 i, const u32* need, const u32* n_gp
     return k;
 }
 
+__device__ __forceinline__ u64 make_k0(u32 i, const u32* need, const u32* n_gpu, const u64* arrival, u32 policy) {
+    if (policy == 2) return arrival[i];
+    const u32 d = need[i], g = n_gpu[i];
+    const u64 a = d > g ? d - g : 0;
+    const u64 inv = 0xFFFFFFFFull - g;
+    return policy == 0 ? (a << 32) | inv : (inv << 32) | a;
+}
+
 __global__ void __launch_bounds__(CWS_THREADS)
     schedule_kernel(u32 R, const u32* __restrict__ need, const u32* __restrict__ n_gpu,
                     const u64* __restrict__ arrival, const u32* __restrict__ req_id, u32 policy, u32 free_blocks,
                     u32 evictable, u32 max_admit, u32* order, u32* a_sorted, u32* ticket, u32* num_admit,
                     u32* deficit) {
-    __shared__ u64 s_k0[CWS_TILE], s_k1[CWS_TILE], s_k2[CWS_TILE];
+    extern __shared__ __align__(16) u64 s_k0[];  // leading words of up to CWS_TILE keys
     __shared__ u64 s_warp[CWS_THREADS / 32];
     __shared__ u32 s_last;
     __shared__ u32 s_count;
     __shared__ unsigned long long s_need;
     const u32 tid = threadIdx.x;
-    const u32 il = tid / CWS_J_LANES, jl = tid % CWS_J_LANES;  // the J_LANES threads of one element are adjacent
+    const u32 il = tid / CWS_J_LANES, jl = tid % CWS_J_LANES;  // one warp per element
     const u32 i = blockIdx.x * CWS_I_PER_CTA + il;
     const bool live = i < R;
     Key3 mine{~0ull, ~0ull, ~0ull};
     if (live) mine = make_key(i, need, n_gpu, arrival, req_id, policy);
 
+    // Per tile of keys: pass 1 (branch-free) counts the leading words that are smaller / equal — the leading word
+    // decides almost every pair; pass 2 runs only if another key of the tile shares this element's leading word and
+    // lets the remaining words (read from global memory: rare) decide among those.
     u32 rank = 0;
     for (u32 base = 0; base < R; base += CWS_TILE) {
         const u32 n = min((u32)CWS_TILE, R - base);
         __syncthreads();
-        for (u32 t = tid; t < n; t += CWS_THREADS) {
-            const Key3 k = make_key(base + t, need, n_gpu, arrival, req_id, policy);
-            s_k0[t] = k.k0;
-            s_k1[t] = k.k1;
-            s_k2[t] = k.k2;
+        for (u32 t0 = tid; t0 < n; t0 += CWS_THREADS * 8) {  // 8 keys per thread in flight: one load latency, not 8
+            u64 v[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const u32 t = t0 + k * CWS_THREADS;
+                v[k] = t < n ? make_k0(base + t, need, n_gpu, arrival, policy) : 0ull;
+            }
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const u32 t = t0 + k * CWS_THREADS;
+                if (t < n) s_k0[t] = v[k];
+            }
         }
         __syncthreads();
+        u32 ties = 0;
         if (live) {
-#pragma unroll 4
+#pragma unroll 8
             for (u32 t = jl; t < n; t += CWS_J_LANES) {
                 const u64 o0 = s_k0[t];
-                if (o0 != mine.k0) {  // decided by the leading word (the common case): 1 load, 2 compares
-                    rank += o0 < mine.k0 ? 1u : 0u;
-                } else {
-                    const Key3 o{o0, s_k1[t], s_k2[t]};
-                    rank += key_less(o, mine) ? 1u : 0u;
-                }
+                rank += o0 < mine.k0 ? 1u : 0u;
+                ties += o0 == mine.k0 ? 1u : 0u;
+            }
+        }
+        ties = __reduce_add_sync(0xffffffffu, ties);  // the lanes of a warp share one element
+        const u32 self = (live && i >= base && i < base + n) ? 1u : 0u;
+        if (ties > self) {
+            for (u32 t = jl; t < n; t += CWS_J_LANES) {
+                const u32 jdx = base + t;
+                if (s_k0[t] != mine.k0 || jdx == i) continue;
+                const u64 o1 = policy == 2 ? 0ull : arrival[jdx];
+                const u64 o2 = ((u64)req_id[jdx] << 32) | jdx;
+                rank += (o1 < mine.k1 || (o1 == mine.k1 && o2 < mine.k2)) ? 1u : 0u;
             }
         }
     }
-#pragma unroll
-    for (int m = 1; m < CWS_J_LANES; m <<= 1) rank += __shfl_xor_sync(0xffffffffu, rank, m);
+    rank = __reduce_add_sync(0xffffffffu, rank);
     if (live && jl == 0) {
         order[rank] = i;
         const u32 d = need[i], g = n_gpu[i];
@@ -168,7 +190,13 @@ int32_t cwi_schedule(cw_ctx* ctx, u32 R, const u32* d_need, const u32* d_n_gpu, 
         return CW_OK;
     }
     const u32 grid = (R + CWS_I_PER_CTA - 1) / CWS_I_PER_CTA;
-    schedule_kernel<<<grid, CWS_THREADS, 0, ctx->s_main>>>(R, d_need, d_n_gpu, d_arrival_seq, d_req_id, policy,
+    static bool attr_set = false;
+    if (!attr_set) {
+        CW_CUDA(ctx, cudaFuncSetAttribute(schedule_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CWS_TILE * 8));
+        attr_set = true;
+    }
+    const size_t smem = (size_t)(R < CWS_TILE ? R : CWS_TILE) * 8;
+    schedule_kernel<<<grid, CWS_THREADS, smem, ctx->s_main>>>(R, d_need, d_n_gpu, d_arrival_seq, d_req_id, policy,
                                                            free_blocks, evictable, max_admit, d_order, ctx->sched_a,
                                                            ctx->sched_ticket, d_num_admit, d_deficit);
     CW_LAUNCH_CHECK(ctx);

@@ -168,6 +168,23 @@ def test_schedule_random_queues(policy):
     ctx.close()
 
 
+def test_schedule_more_requests_than_one_key_tile():
+    """R > 8192: the leading key words are staged tile by tile; heavy ties force the second pass in every tile."""
+    from gpu_util import small_ctx
+    R = 20000
+    ctx = small_ctx(max_requests=R)
+    g = gen.rng(24, 0)
+    for policy in (0, 1, 2):
+        d = g.integers(0, 20, size=R).astype(np.uint32)
+        n_gpu = np.minimum(d, g.integers(0, 20, size=R)).astype(np.uint32)
+        arr = g.integers(0, 50, size=R).astype(np.uint64)
+        rid = g.integers(0, 100, size=R).astype(np.uint32)
+        eo, ena, ede = oracle.schedule(d, n_gpu, arr, rid, policy, 1000, 50000, R)
+        o, na, de = _schedule(ctx, d, n_gpu, arr, rid, policy, 1000, 50000, R)
+        assert (o == eo).all() and (na, de) == (ena, ede), policy
+    ctx.close()
+
+
 def test_schedule_edges():
     import paper_2606_16824_b200 as cw
     from gpu_util import small_ctx

@@ -11,8 +11,9 @@
 //          of equal length, one per CTA.  A CTA therefore walks its requests sequentially and never waits on
 //          another CTA (no look-back, no spinning).  Only the first request of a range can have begun in an
 //          earlier range: that boundary segment is scanned with carry-in 0 and patched at the very end of the
-//          CTA, H_j += A^(j-j0+1) * carry_in (linear in the carry, mod 2^64), once the CTA of the previous
-//          range has published its final chain state.  Ranges are handed out by an atomic ticket, so the
+//          CTA, H_j += A^(j-j0+1) * carry_in (linear in the carry, mod 2^64), from the chain states the CTAs of the
+//          earlier ranges have published (a range wholly inside one request publishes its carry-free tail and
+//          its length, and the reader folds those while walking back).  Ranges are handed out by an atomic ticket, so the
 //          CTA that is waited for has always started: the single wait per CTA cannot deadlock and happens
 //          when both CTAs are finishing anyway.
 //
@@ -353,21 +354,25 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, 4) hash_kernel(const HashArgs a
     const u32 flags = sm.rec_flags;
     const u32 bseg_len = sm.rec_bseg_len;
     if (tid == 0) {
-        const bool dependent = (flags & CWH_REC_TAIL_IS_BSEG) != 0;  // whole range inside one request
-        if (!dependent) {  // the tail is already final: publish before waiting, so waits never chain
-            a.rec[range].true_tail = sm.rec_tail_state;
-            st_release_u32(&a.rec[range].ready, epoch);
-        }
+        // Publish at once, never after a wait: a range that lies wholly inside one request publishes its CARRY-FREE
+        // tail together with its length; the reader folds such records while walking back to the first final one
+        // (decoupled look-back over ranges: every CTA walks on its own, nobody waits for a chain of CTAs).
+        const bool dependent = (flags & CWH_REC_TAIL_IS_BSEG) != 0;
+        a.rec[range].tail = sm.rec_tail_state;
+        a.rec[range].len_kind = dependent ? (bseg_len | 0x80000000u) : 0u;
+        st_release_u32(&a.rec[range].ready, epoch);
         u64 carry_in = 0;
         if (flags & CWH_REC_MID) {  // the true chain state at the end of the previous range
-            const cw_hash_rec* prev = a.rec + (range - 1);
-            while (ld_acquire_u32(&prev->ready) != epoch) {
+            u64 mult = 1;
+            for (u32 k = range; k-- > 0;) {
+                const cw_hash_rec* prev = a.rec + k;
+                while (ld_acquire_u32(&prev->ready) != epoch) {
+                }
+                carry_in += mult * ld_relaxed_u64(&prev->tail);
+                const u32 lk = *reinterpret_cast<const volatile u32*>(&prev->len_kind);
+                if (!(lk & 0x80000000u)) break;  // a final tail: the walk ends (range 0 is always final)
+                mult *= pow_u64(CW_A, lk & 0x7FFFFFFFu);
             }
-            carry_in = ld_relaxed_u64(&prev->true_tail);
-        }
-        if (dependent) {
-            a.rec[range].true_tail = sm.rec_tail_state + pow_u64(CW_A, bseg_len) * carry_in;
-            st_release_u32(&a.rec[range].ready, epoch);
         }
         sm.carry_in = carry_in;
     }

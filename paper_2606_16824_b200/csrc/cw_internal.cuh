@@ -65,9 +65,9 @@ __host__ __device__ __forceinline__ u64 cw_remap_key(u64 k) {
 #define CWH_STAGE_BYTES (CWH_UNIT * 64 + 16)
 
 struct cw_hash_rec {  // what the CTA of one range publishes for the CTA of the next range
-    u64 true_tail;  // chain state after the last block of the range
-    u32 ready;      // == call epoch once true_tail is final
-    u32 pad;
+    u64 tail;      // chain state after the last block of the range (carry-free if the range is "dependent")
+    u32 ready;     // == call epoch once the record is published
+    u32 len_kind;  // bit 31: dependent (the whole range lies inside one request begun earlier); low bits: its blocks
 };
 #define CWH_REC_MID 1u           // the range starts in the middle of a request
 #define CWH_REC_TAIL_IS_BSEG 2u  // the whole range lies inside that request

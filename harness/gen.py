@@ -139,6 +139,7 @@ class Turn:
     gap_ms: int          # tool / think time after this turn completes, before the next request arrives
     features: np.ndarray  # uint8[F] tool-call metadata features attached when the turn completes
     true_tau_ms: int     # = gap_ms (ground truth for the CacheWise* "Hint" override)
+    cluster: int = 0     # metadata cluster of the tool call that follows this turn (paper predictor, L227)
 
 
 @dataclass
@@ -190,6 +191,41 @@ def session_trace(seed: int, n_sessions: int, n_turns: int, F: int, init_len, gr
     gw = rng(seed, 999)
     weights[1:] = gw.integers(-8, 9, size=F - 1).astype(np.int16)
     return Trace(sessions, weights, -20000, F, dict(seed=seed, n_sessions=n_sessions, n_turns=n_turns))
+
+
+def tool_clusters(seed: int, C: int = 20, n_lo: int = 9, n_hi: int = 64):
+    """Synthetic per-cluster tool-duration history, shaped like PAPER.md Table 3 (L241-248) / Fig. 9 (L137-169):
+    cluster medians log-spaced from ~50 ms to ~80 s, heavy right tails (P90/P50 between 2x and ~100x), 9..64 samples
+    per cluster.  Returns (median_ms[C], sigma[C], sample_off u64[C+1], samples u32[sum n], sorted inside a cluster)."""
+    g = rng(seed, 500)
+    med = np.exp(np.linspace(np.log(50.0), np.log(80000.0), C))
+    sig = g.uniform(0.5, 2.0, size=C)
+    n = g.integers(n_lo, n_hi + 1, size=C)
+    off = np.zeros(C + 1, np.uint64)
+    np.cumsum(n, out=off[1:].view(np.int64))
+    samples = np.concatenate([np.sort(lognormal_int(g, med[c], sig[c], 1, 10_000_000, size=int(n[c]))) for c in range(C)])
+    return med, sig, off, samples.astype(np.uint32)
+
+
+def cluster_trace(seed: int, n_sessions: int, n_turns: int, C: int = 20, init_len=(6000.0, 0.6, 1024, 24000),
+                  grow_lo: int = 128, grow_hi: int = 1024, cap: int = 40000) -> Trace:
+    """Sessions whose tool gaps are drawn from the per-cluster distributions of tool_clusters(seed): every turn ends
+    with a tool call of a random cluster (fast clusters more often, as in Fig. 9), whose duration is a fresh draw from
+    that cluster's lognormal — the replay only sees the cluster id and the HISTORICAL samples (a separate draw)."""
+    med, sig, off, samples = tool_clusters(seed, C)
+    tr = session_trace(seed, n_sessions, n_turns, 8, init_len, grow_lo, grow_hi, 1.0, cap, [(1.0, 1000.0, 1.0)])
+    w = 1.0 / np.arange(1, C + 1)
+    w /= w.sum()
+    for s, turns in enumerate(tr.sessions):
+        g = rng(seed, 700 + s)
+        for t in turns:
+            c = int(g.choice(C, p=w))
+            t.cluster = c
+            t.gap_ms = int(lognormal_int(g, med[c], sig[c], 1, 10_000_000))
+            t.true_tau_ms = t.gap_ms
+            t.features[0] = min(255, int(np.log2(t.gap_ms + 1) * 10))  # the linear predictor's proxy feature
+    tr.meta.update(sample_off=off, samples=samples, C=C)
+    return tr
 
 
 def tiny_trace(seed: int = 0) -> Trace:

@@ -38,7 +38,8 @@ class ReplayConfig:
     max_admit: int = 2
     use_hint: bool = False          # CacheWise* (PAPER.md L285): tau_override = true gap
     evict_policy: str = "cachewise"  # "cachewise" (per-session linear predictor), "hint" (= use_hint), "lru" (vLLM,
-                                     # L281: every tau equal), "infercept" (L283: session moving average of tool time)
+                                     # L281: every tau equal), "infercept" (L283: session moving average of tool time),
+                                     # "cluster" (the paper's predictor, L219-227: cw_predict_tau over per-cluster history)
     c0_ms: int = 20                 # integer service model: c0 + ceil(c_tok*new_tokens/1000) + c_blk*swapped_in
     c_tok_us: int = 250
     c_blk_ms: int = 1
@@ -144,6 +145,7 @@ def run(trace: gen.Trace, cfg: ReplayConfig, be) -> ReplayResult:
     now, tick, seq, rid = 0, 1, 0, 0
     gap_avg = np.zeros(S, np.int64)      # InferCept baseline: what the session's tool calls took so far
     last_done = np.zeros(S, np.int64)
+    sess_cluster = np.zeros(S, np.uint32)  # cluster of the tool call each session is waiting on
 
     def flags(ids):
         return (np.where(b_valid[ids], REF_VALID, 0) | b_ref[ids]).astype(np.uint32)
@@ -246,6 +248,9 @@ def run(trace: gen.Trace, cfg: ReplayConfig, be) -> ReplayResult:
                 tau_ov = np.clip(next_arrival - now, 0, 0xFFFFFF).astype(np.uint32)
             elif cfg.evict_policy == "lru":
                 tau_ov = np.full(S, 1000, np.uint32)
+            elif cfg.evict_policy == "cluster":     # E[remaining | still running] from the cluster's history
+                tau_ov = be.predict_tau(sess_cluster, np.clip(now - last_done, 0, 0xFFFFFFFF).astype(np.uint32),
+                                        trace.meta["sample_off"], trace.meta["samples"])
             elif cfg.evict_policy == "infercept":   # moving average of the session's past gaps minus the elapsed time
                 tau_ov = np.clip(gap_avg - (now - last_done), 0, 0xFFFFFF).astype(np.uint32)
             victims, vscores, st = be.score_evict(tick, features, trace.weights, trace.bias, state, tau_ov, short, 0,
@@ -363,6 +368,7 @@ def run(trace: gen.Trace, cfg: ReplayConfig, be) -> ReplayResult:
                 state[s] = gen.TOOL_WAIT
                 next_arrival[s] = now + t.gap_ms
                 last_done[s] = now
+                sess_cluster[s] = t.cluster
                 if q.turn > 0:  # the previous gap is known by now: exponential moving average (alpha = 1/2)
                     prev_gap = trace.sessions[s][q.turn - 1].gap_ms
                     gap_avg[s] = prev_gap if q.turn == 1 else (gap_avg[s] + prev_gap) // 2
@@ -385,6 +391,7 @@ SYSTEMS = {  # the paper's comparison systems as (schedule policy, eviction poli
     "InferCept (FCFS + moving average)": (2, "infercept"),
     "vLLM (prefix-aware)": (0, "lru"),
     "CacheWise (prefix-aware + predictor)": (0, "cachewise"),
+    "CacheWise (prefix-aware + cluster predictor)": (0, "cluster"),
     "CacheWise* (prefix-aware + true tau)": (0, "hint"),
 }
 
@@ -394,6 +401,8 @@ def policy_sweep(trace: gen.Trace, base: ReplayConfig, make_backend):
     import dataclasses
     out = {}
     for name, (sched, ev) in SYSTEMS.items():
+        if ev == "cluster" and "samples" not in trace.meta:
+            continue
         cfg = dataclasses.replace(base, policy=sched, evict_policy=ev, use_hint=False)
         r = run(trace, cfg, make_backend(cfg))
         t = r.totals()
@@ -536,6 +545,15 @@ class GpuBackend:
             return tier[slots.astype(np.int64)].reshape(-1).copy()
         return np.zeros(0, np.uint8)
 
+    def predict_tau(self, cluster, elapsed_ms, sample_off, samples):
+        t = self.torch
+        with t.cuda.stream(self.stream):
+            d_out = t.zeros(cluster.size, dtype=t.int32, device="cuda")
+            self.ctx.predict_tau(cluster.size, self._dev(cluster, np.uint32), self._dev(elapsed_ms, np.uint32),
+                                 sample_off.size - 1, self._dev(sample_off, np.uint64), self._dev(samples, np.uint32), d_out)
+            self.ctx.sync()
+            return self.st.host(d_out, np.uint32)
+
     def swap_in(self, slots, dst):
         with self.torch.cuda.stream(self.stream):
             self.ctx.swap_in(np.ascontiguousarray(slots, np.uint32), self.tier, self._dev(dst, np.uint32), dst.size)
@@ -607,8 +625,7 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="run the paper's comparison systems on a synthetic trace")
     a = ap.parse_args()
     if a.sweep:
-        tr = gen.session_trace(21, 48, 24, 8, (6000.0, 0.6, 1024, 24000), 128, 1024, 1.0, 40000,
-                               [(0.7, 1000.0, 1.0), (0.3, 60000.0, 1.0)])
+        tr = gen.cluster_trace(31, 48, 24)   # tool gaps drawn from 20 per-cluster distributions (Table 3 shaped)
         ws = sum(max((t.tokens.size + 15) // 16 for t in s) for s in tr.sessions)
         base = ReplayConfig("sweep", int(0.3 * ws), 0, 4, 4096, max_admit=8, store_bytes=False)
         print(json.dumps(policy_sweep(tr, base, lambda c: GpuBackend(c, 48, 8)), indent=1))

@@ -147,6 +147,18 @@ int32_t cw_score_evict(cw_ctx* ctx, uint32_t tick_now, uint32_t S, uint32_t F, c
                        const uint32_t* d_tau_override, const uint32_t* d_deficit, uint32_t tier,
                        uint32_t* d_victims, uint64_t* d_victim_scores, uint32_t* d_num_victims, uint32_t cap);
 
+/* The paper's own predictor (PAPER.md 5.2 L219-225 "expected remaining time for the tool call to complete",
+ * L227 per-cluster distributions of historical tool durations).  DESIGN.md reading R7.
+ *   d_cluster    uint32[S]: cluster of the tool call each session is waiting on (its metadata class)
+ *   d_elapsed_ms uint32[S]: t - T_i, time since that call was issued
+ *   d_sample_off uint64[C+1], d_samples uint32[sample_off[C]]: historical durations (ms) of every cluster, ASCENDING
+ *                inside a cluster
+ *   d_tau_out    uint32[S]: clamp(floor(mean of the cluster's samples > elapsed) - elapsed, 0, CW_TAU_MAX-1); if no
+ *                sample exceeds elapsed (or the cluster is empty): min(elapsed, CW_TAU_MAX-1)
+ * The result is meant for cw_score_evict's d_tau_override.  cluster >= C -> tau 0 and CW_E_INVAL at cw_sync. */
+int32_t cw_predict_tau(cw_ctx* ctx, uint32_t S, const uint32_t* d_cluster, const uint32_t* d_elapsed_ms, uint32_t C,
+                       const uint64_t* d_sample_off, const uint32_t* d_samples, uint32_t* d_tau_out);
+
 /* Stage 4 — paged KV swap (PAPER.md 6.4 L345 "transferred from GPU memory to CPU DRAM and swapped back on
  * demand", Fig. 18).  DESIGN.md reading R5.  A staged page = chunks 0..n_chunks-1 contiguous.
  *

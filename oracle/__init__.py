@@ -207,3 +207,13 @@ def swap_in(pool, n_chunks, chunk_bytes, chunk_stride, block_stride, src, dst_bl
     lib().cwo_swap_in(_p(pool), C.c_uint32(n_chunks), C.c_uint64(chunk_bytes), C.c_uint64(chunk_stride),
                       C.c_uint64(block_stride), _p(slots), _p(src), _p(dst_blocks), C.c_uint32(dst_blocks.size))
     return pool
+
+
+def predict_tau(cluster, elapsed_ms, sample_off, samples):
+    """Paper predictor (R7).  Returns (tau u32[S], status)."""
+    cluster, elapsed_ms = _arr(cluster, np.uint32), _arr(elapsed_ms, np.uint32)
+    sample_off, samples = _arr(sample_off, np.uint64), _arr(samples, np.uint32)
+    tau = np.empty(cluster.size, np.uint32)
+    st = lib().cwo_predict_tau(C.c_uint32(cluster.size), _p(cluster), _p(elapsed_ms), C.c_uint32(sample_off.size - 1),
+                               _p(sample_off), _p(samples), _p(tau))
+    return tau, st

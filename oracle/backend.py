@@ -70,6 +70,9 @@ class OracleBackend:
             return self.tier.reshape(-1, c.page)[slots.astype(np.int64)].reshape(-1).copy()
         return np.zeros(0, np.uint8)
 
+    def predict_tau(self, cluster, elapsed_ms, sample_off, samples):
+        return oracle.predict_tau(cluster, elapsed_ms, sample_off, samples)[0]
+
     def swap_in(self, slots, dst):
         if self.pool is None:
             return

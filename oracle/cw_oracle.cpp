@@ -315,4 +315,36 @@ int cwo_swap_in(uint8_t* pool, u32 n_chunks, u64 chunk_bytes, u64 chunk_stride, 
     return 0;
 }
 
+// ------------------------------------------------------------------------------------------------
+// NEXT-1 — the paper's own predictor.  PAPER.md 5.2 L219-225: "at time t, CacheWise estimates
+// the expected remaining time for the tool call to complete, i.e. E[tau_i(t) | tau_i(t) - T_i > t - T_i], by
+// analyzing distributions of tool execution durations with similar metadata m"; L227: per-cluster empirical
+// distributions.  DESIGN.md reading R7: with the historical durations d_0..d_{n-1} (ms) of the session's
+// cluster and the elapsed time e = t - T_i,
+//     tau = clamp( floor( sum_{d_k > e} d_k / #{d_k > e} ) - e , 0, TAU_MAX-1 )
+// and, when no historical call of the cluster ran longer than e (or the cluster is empty), tau = min(e,
+// TAU_MAX-1) (the call has outlived all history: expect it to take as long again).  cluster >= C -> tau = 0, status -1.
+// ------------------------------------------------------------------------------------------------
+int cwo_predict_tau(u32 S, const u32* cluster, const u32* elapsed_ms, u32 C, const u64* sample_off,
+                    const u32* samples, u32* tau_out) {
+    int status = 0;
+    for (u32 s = 0; s < S; ++s) {
+        u32 c = cluster[s];
+        if (c >= C) {
+            tau_out[s] = 0;
+            status = -1;
+            continue;
+        }
+        u64 e = elapsed_ms[s], sum = 0, cnt = 0;
+        for (u64 k = sample_off[c]; k < sample_off[c + 1]; ++k)
+            if (samples[k] > e) {
+                sum += samples[k];
+                ++cnt;
+            }
+        u64 tau = cnt ? sum / cnt - e : e;
+        tau_out[s] = (u32)std::min<u64>(tau, TAU_MAX - 1);
+    }
+    return status;
+}
+
 }  // extern "C"

@@ -22,7 +22,7 @@ CW_REF_PINNED = 0x40000000
 POLICY_MIN_ADDITIONAL, POLICY_OVERLAP_FIRST, POLICY_FCFS = 0, 1, 2
 
 EXPORTS = ["cw_create", "cw_destroy", "cw_sync", "cw_join_copy", "cw_debug_evict_times", "cw_last_error", "cw_launch_count", "cw_hash_blocks",
-           "cw_match_prefix", "cw_schedule", "cw_score_evict", "cw_swap_out", "cw_swap_in", "cw_gather_pages",
+           "cw_match_prefix", "cw_schedule", "cw_score_evict", "cw_predict_tau", "cw_swap_out", "cw_swap_in", "cw_gather_pages",
            "cw_scatter_pages", "cw_table_insert", "cw_table_erase", "cw_table_retag", "cw_table_lookup",
            "cw_blocks_update"]
 
@@ -67,6 +67,7 @@ def lib():
         L.cw_match_prefix.argtypes = [P, P, P, U32, P, P, P]
         L.cw_schedule.argtypes = [P, U32, P, P, P, P, U32, U32, U32, U32, P, P, P]
         L.cw_score_evict.argtypes = [P, U32, U32, U32, P, P, I32, P, P, P, U32, P, P, P, U32]
+        L.cw_predict_tau.argtypes = [P, U32, P, P, U32, P, P, P]
         L.cw_swap_out.argtypes = [P, P, P, U32, P, P]
         L.cw_swap_in.argtypes = [P, P, P, P, U32]
         L.cw_gather_pages.argtypes = [P, P, P, U32, P]
@@ -170,6 +171,10 @@ class Context:
         self._ck(lib().cw_score_evict(self._h, tick_now, S, F, _ptr(features), _ptr(weights), bias,
                                       _ptr(session_state), _ptr(tau_override), _ptr(deficit), tier, _ptr(victims),
                                       _ptr(victim_scores), _ptr(num_victims), cap), "cw_score_evict")
+
+    def predict_tau(self, S, cluster, elapsed_ms, C, sample_off, samples, tau_out):
+        self._ck(lib().cw_predict_tau(self._h, S, _ptr(cluster), _ptr(elapsed_ms), C, _ptr(sample_off), _ptr(samples),
+                                      _ptr(tau_out)), "cw_predict_tau")
 
     def swap_out(self, victims, num_victims, cap, host_slots, h_dst):
         self._ck(lib().cw_swap_out(self._h, _ptr(victims), _ptr(num_victims), cap, _ptr(host_slots), _ptr(h_dst)),

@@ -248,6 +248,14 @@ int32_t cw_score_evict(cw_ctx* ctx, uint32_t tick_now, uint32_t S, uint32_t F, c
                            d_deficit, tier, d_victims, d_victim_scores, d_num_victims, cap);
 }
 
+int32_t cw_predict_tau(cw_ctx* ctx, uint32_t S, const uint32_t* d_cluster, const uint32_t* d_elapsed_ms, uint32_t C,
+                       const uint64_t* d_sample_off, const uint32_t* d_samples, uint32_t* d_tau_out) {
+    if (!ctx) return CW_E_STATE;
+    if (S == 0) return CW_OK;
+    if (!d_cluster || !d_elapsed_ms || !d_sample_off || !d_tau_out || (C && !d_samples)) return CW_E_INVAL;
+    return cwi_predict_tau(ctx, S, d_cluster, d_elapsed_ms, C, d_sample_off, d_samples, d_tau_out);
+}
+
 int32_t cw_gather_pages(cw_ctx* ctx, const uint32_t* d_ids, const uint32_t* d_num, uint32_t cap, void* d_staged) {
     if (!ctx) return CW_E_STATE;
     if (!ctx->cfg.n_chunks) return CW_E_STATE;

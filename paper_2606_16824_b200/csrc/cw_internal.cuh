@@ -273,5 +273,6 @@ int32_t cwi_score_evict(cw_ctx*, u32, u32, u32, const uint8_t*, const int16_t*, 
 int32_t cwi_copy_pages(cw_ctx*, cudaStream_t, const u32* d_ids, const u32* d_num, u32 first, u32 cap, void* d_staged,
                        bool gather);
 int32_t cwi_blocks_update(cw_ctx*, u32, const u32*, u32, const u32*, const u32*, const u32*, const u32*);
+int32_t cwi_predict_tau(cw_ctx*, u32, const u32*, const u32*, u32, const u64*, const u32*, u32*);
 int cwi_hash_grid(int n_sm);
 int cwi_copy_grid(int n_sm);

@@ -4,7 +4,8 @@
 // driving a shared-memory ring with the TMA engine: cp.async.bulk global->shared (mbarrier complete_tx),
 // then cp.async.bulk shared->global (bulk_group), CWC_AHEAD loads in flight ahead of the stores.  No data
 // ever passes through registers.  Work item = (page j, chunk c, piece) of <= CWC_PIECE bytes; items are
-// dealt round-robin to the CTAs so that every SM streams the same amount.
+// dealt round-robin to the CTAs so that every SM streams the same amount.  A block-major pool (chunk_stride ==
+// chunk_bytes: the page is contiguous) is moved as ONE chunk per page, so small chunks still travel in 16 KiB pieces.
 #include <stdio.h>
 
 #include "cw_internal.cuh"

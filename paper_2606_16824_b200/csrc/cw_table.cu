@@ -13,10 +13,12 @@
 // (All same-key threads follow one probe sequence whose slots only go from reusable to occupied during the
 // batch, so they converge on the same slot.)
 //
-// Match: one lane per hash, flat over hashes[]; a warp finds its request by a 32-ary search over hash_off.
-// Per request: first_miss = atomicMin over missing lanes, max_hit = atomicMax over hits that are not
-// already behind a miss of their own warp; a small per-request kernel then writes k_total / n_gpu and
-// blanks hits that lie behind the first miss (rare), and re-arms the scratch for the next call.
+// Match: one lane per hash, flat over hashes[]; a warp task is 256 consecutive hashes (one 32-ary search over
+// hash_off for its first request, then a sequential walk; rounds that lie behind a miss already seen for their
+// request are answered without a probe).  Per request: first_miss = atomicMin over missing lanes, max_hit =
+// atomicMax over hits that are not already behind a miss of their own round; a small per-request kernel then
+// writes k_total / n_gpu and blanks hits that lie behind the first miss (rare), and re-arms the scratch for the
+// next call.
 #include <stdio.h>
 
 #include "cw_internal.cuh"

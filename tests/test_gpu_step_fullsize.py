@@ -62,3 +62,35 @@ def test_full_size_step_matches_the_oracle_everywhere():
     for k in ("hashes", "k_total", "n_gpu", "hit_loc", "order", "victims", "victim_scores"):
         assert np.array_equal(res[k], res2[k]), f"steady step: {k}"
     st.close()
+
+
+def test_repeated_steps_are_deterministic_and_self_cleaning():
+    """300 back-to-back steps (cold / steady alternating, hashes cleared in between) on a 1/16 snapshot must give the
+    same outputs every time: the kernels' scratch (tickets, epochs, histograms, barrier words) cleans itself, and
+    nothing depends on the order in which CTAs or atomics happen to run."""
+    import torch
+
+    from harness import stress
+    snap = gen.stress_snapshot(seed=5, S=16)
+    stream = torch.cuda.Stream()
+    st = stress.StressStep(snap, stream)
+
+    def digest():
+        w = torch.arange(1, st.cap + 1, device="cuda")
+        return (int(st.d_hashes.sum().item()), int(st.d_k.sum().item()), int(st.d_g.sum().item()),
+                int(st.d_loc.to(torch.int64).sum().item()),
+                int((st.d_order.to(torch.int64) * torch.arange(1, st.R + 1, device="cuda")).sum().item()),
+                int((st.d_vic.to(torch.int64) * w).sum().item()), int(st.d_sc.sum().item()), int(st.d_nv.item()),
+                int(st.d_def.item()), int(st.d_na.item()))
+
+    with torch.cuda.stream(stream):
+        st.step()
+        first = digest()
+        assert first[7] > 0
+        for i in range(300):
+            if i % 3 == 0:
+                st.d_hashes.zero_()
+            st.step(steady=(i % 3 == 1))
+            assert digest() == first, i
+    assert st.ctx.sync(check=False) == 0
+    st.close()

@@ -110,7 +110,9 @@ int32_t cw_hash_blocks(cw_ctx* ctx, const int32_t* d_tokens, const uint64_t* d_t
  * prefix, Fig. 11B "overlap with KVCache resident on the XPU").  DESIGN.md reading R2.
  *   d_k_total uint32[R]: length of the LEADING run of resident hashes (either tier)
  *   d_n_gpu   uint32[R]: how many blocks of that run are in HBM (= the paper's k_i)
- *   d_hit_loc uint32[hash_off[R]] or NULL: loc of each block of the run; CW_MISS from the first miss on */
+ *   d_hit_loc uint32[hash_off[R]] or NULL: loc of each block of the run; CW_MISS from the first miss on
+ * hash_off may be a slice of a longer CSR array (absolute offsets); at most 2^32-1 hashes per call (more ->
+ * CW_E_INVAL at cw_sync, outputs untouched). */
 int32_t cw_match_prefix(cw_ctx* ctx, const uint64_t* d_hashes, const uint64_t* d_hash_off, uint32_t R,
                         uint32_t* d_k_total, uint32_t* d_n_gpu, uint32_t* d_hit_loc);
 

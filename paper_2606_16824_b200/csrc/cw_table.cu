@@ -182,68 +182,77 @@ __global__ void insert_reset_kernel(cw_slot* table, u32 n, const u32* ins_slot) 
                        // configs[2] (128: 97 us, 256: 100, 512: 105, 1024: 124, 2048: 208 — long tasks are bound by the
                        // dependent probe chain of the slowest warp, short ones by occupancy x latency)
 
-__global__ void __launch_bounds__(256, MATCH_MIN_CTAS) match_probe_kernel(const cw_slot* __restrict__ table, u64 mask,
+__global__ void __launch_bounds__(256, MATCH_MIN_CTAS) match_probe_kernel(const cw_slot* __restrict__ table, u32 mask,
                                                           const u64* __restrict__ hashes,
                                                           const u64* __restrict__ hash_off, u32 R, u32* first_miss,
-                                                          u32* max_hit, u32* host_hits, u32* hit_loc) {
-    const u64 h_first = hash_off[0], total = hash_off[R];  // hash_off may be a slice of a longer CSR array
+                                                          u32* max_hit, u32* host_hits, u32* hit_loc, u32* status) {
+    // hash_off may be a slice of a longer CSR array: positions below are 32-bit offsets from its first hash
+    const u64 h_first = hash_off[0];
+    if (hash_off[R] - h_first > 0xFFFFFFFFull) {  // more than 2^32 hashes in one call: not supported
+        if (blockIdx.x == 0 && threadIdx.x == 0) atomicOr(status, CWS_INVAL);
+        return;
+    }
+    const u32 total = (u32)(hash_off[R] - h_first);
+    const u64* __restrict__ hs = hashes + h_first;
+    u32* hl = hit_loc ? hit_loc + h_first : nullptr;
     const u32 lane = threadIdx.x & 31;
-    const u64 nwarps = ((u64)gridDim.x * blockDim.x) >> 5;
+    const u32 nwarps = (gridDim.x * blockDim.x) >> 5;
+    const u32 n_tasks = (total + CWM_CHUNK - 1) / CWM_CHUNK;
     // a warp walks its task front to back, so once it has seen a miss of a request the rest of that request is
     // answered without touching the table (the leading run is over); a miss recorded by an earlier task of the
     // same request is honoured too when the warp enters that request
-    for (u64 w = ((u64)blockIdx.x * blockDim.x + threadIdx.x) >> 5; h_first + w * CWM_CHUNK < total; w += nwarps) {
-        const u64 c0 = h_first + w * CWM_CHUNK;
+    for (u32 w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; w < n_tasks; w += nwarps) {
+        const u32 c0 = w * CWM_CHUNK;
         // largest r with hash_off[r] <= c0 (r < R), 32-ary search, warp-uniform, once per task
         u32 lo = 0, hi = R;
         while (hi - lo > 1) {
             u32 step = (hi - lo + 31) >> 5;
             u32 p = lo + lane * step;
-            bool ok = p < hi && hash_off[p] <= c0;
+            bool ok = p < hi && (u32)(hash_off[p] - h_first) <= c0;
             u32 cnt = __popc(__ballot_sync(0xffffffffu, ok));
             u32 nlo = lo + (cnt - 1) * step;
             hi = min(hi, nlo + step);
             lo = nlo;
         }
         u32 r_base = lo;  // request of the first hash of the current round (kept up to date below)
-        u64 req_start = hash_off[lo], req_end = hash_off[lo + 1];
+        u32 req_start = (u32)(hash_off[lo] - h_first), req_end = (u32)(hash_off[lo + 1] - h_first);
         u32 dead_r = 0xFFFFFFFFu, checked_r = 0xFFFFFFFFu;  // request known to have missed / whose global state was read
-        const u64 c1 = min(total, c0 + CWM_CHUNK);
-        u64 key_next = c0 + lane < c1 ? hashes[c0 + lane] : 0;
-        for (u64 g0 = c0; g0 < c1; g0 += 32) {
+        const u32 c1 = min(total, c0 + CWM_CHUNK);
+        u64 key_next = c0 + lane < c1 ? hs[c0 + lane] : 0;
+        for (u32 g0 = c0; g0 < c1; g0 += 32) {
             while (g0 >= req_end) {  // warp-uniform; also skips empty requests
                 ++r_base;
                 req_start = req_end;
-                req_end = hash_off[r_base + 1];
+                req_end = (u32)(hash_off[r_base + 1] - h_first);
             }
-            const u64 g = g0 + lane;
+            const u32 g = g0 + lane;
             const bool active = g < c1;
             const u64 key = key_next;
-            if (g + 32 < c1) key_next = hashes[g + 32];  // prefetch the next round
+            if (g + 32 < c1) key_next = hs[g + 32];  // prefetch the next round
             u32 r = r_base;
-            u32 j = (u32)(g - req_start);
+            u32 j = g - req_start;
             bool uniform = true;
             if (min(g0 + 32, c1) > req_end) {  // the round crosses into the next request(s): per-lane walk (rare)
                 if (active)
-                    while (g >= hash_off[r + 1]) ++r;
-                j = active ? (u32)(g - hash_off[r]) : 0;
+                    while (g >= (u32)(hash_off[r + 1] - h_first)) ++r;
+                j = active ? g - (u32)(hash_off[r] - h_first) : 0;
                 uniform = __all_sync(0xffffffffu, !active || r == r_base);
             }
-            const u32 act_mask = __ballot_sync(0xffffffffu, active);
             if (uniform) {
                 if (r_base != checked_r && r_base != dead_r) {  // entering a request: did an earlier task miss?
                     checked_r = r_base;
-                    const u32 j0 = (u32)(g0 - hash_off[r_base]);
+                    const u32 j0 = g0 - req_start;
                     if (j0 > 0 && __ldcg(first_miss + r_base) < j0) dead_r = r_base;
                 }
                 if (r_base == dead_r) {  // the whole round lies behind a known miss
-                    if (active && hit_loc) hit_loc[g] = CW_MISS;
+                    if (active && hl) hl[g] = CW_MISS;
                     continue;
                 }
             }
             u32 loc = CW_MISS;
-            if (active) loc = table_probe(table, (u32)mask, cw_remap_key(key));
+            if (active) loc = table_probe(table, mask, cw_remap_key(key));
             if (uniform) {
+                const u32 act_mask = __ballot_sync(0xffffffffu, active);
                 const u32 miss_mask = __ballot_sync(0xffffffffu, active && loc == CW_MISS);
                 const u32 first = miss_mask ? (u32)__ffs(miss_mask) - 1 : 32;
                 if (lane > first) loc = CW_MISS;
@@ -263,7 +272,7 @@ __global__ void __launch_bounds__(256, MATCH_MIN_CTAS) match_probe_kernel(const 
                     if (loc & CW_HOST_BIT) atomicAdd(&host_hits[r], 1u);
                 }
             }
-            if (active && hit_loc) hit_loc[g] = loc;
+            if (active && hl) hl[g] = loc;
         }
     }
 }
@@ -371,9 +380,9 @@ int32_t cwi_match_prefix(cw_ctx* ctx, const u64* d_hashes, const u64* d_hash_off
     u64 cap = (u64)ctx->n_sm * 8 * 4;
     if (blocks > cap) blocks = cap;
     if (blocks < 1) blocks = 1;
-    match_probe_kernel<<<(u32)blocks, 256, 0, ctx->s_main>>>(ctx->table, mask, d_hashes, d_hash_off, R,
+    match_probe_kernel<<<(u32)blocks, 256, 0, ctx->s_main>>>(ctx->table, (u32)mask, d_hashes, d_hash_off, R,
                                                              ctx->m_first_miss, ctx->m_max_hit, ctx->m_host_hits,
-                                                             d_hit_loc);
+                                                             d_hit_loc, ctx->d_status);
     CW_LAUNCH_CHECK(ctx);
     match_finish_kernel<<<cdiv((u64)R * 32, 256), 256, 0, ctx->s_main>>>(d_hash_off, R, ctx->m_first_miss,
                                                                          ctx->m_max_hit, ctx->m_host_hits, d_k_total,

@@ -13,7 +13,7 @@
 // (All same-key threads follow one probe sequence whose slots only go from reusable to occupied during the
 // batch, so they converge on the same slot.)
 //
-// Match: one lane per hash, flat over hashes[]; a warp task is 256 consecutive hashes (one 32-ary search over
+// Match: one lane per hash, flat over hashes[]; a warp task is 128 consecutive hashes (one 32-ary search over
 // hash_off for its first request, then a sequential walk; rounds that lie behind a miss already seen for their
 // request are answered without a probe).  Per request: first_miss = atomicMin over missing lanes, max_hit =
 // atomicMax over hits that are not already behind a miss of their own round; a small per-request kernel then
@@ -178,9 +178,9 @@ __global__ void insert_reset_kernel(cw_slot* table, u32 n, const u32* ins_slot) 
 // 8 CTAs of 256 threads per SM (<= 32 registers): the probe is bound by resident warps x latency (93 us vs 107 us
 // at 6 CTAs/SM on configs[2])
 #define MATCH_MIN_CTAS 8
-#define CWM_CHUNK 256  // consecutive hashes handled by one warp task (8 rounds of 32): measured optimum on
-                       // configs[2] (128: 97 us, 256: 100, 512: 105, 1024: 124, 2048: 208 — long tasks are bound by the
-                       // dependent probe chain of the slowest warp, short ones by occupancy x latency)
+#define CWM_CHUNK 128  // consecutive hashes handled by one warp task (4 rounds of 32): measured optimum on configs[2]
+                       // (64: 89 us, 128: 75, 256: 79, 512: ~85, 1024: ~100, 2048: ~170 — long tasks are bound by the
+                       // dependent probe chain of the slowest warp, short ones by the per-task search and set-up)
 
 __global__ void __launch_bounds__(256, MATCH_MIN_CTAS) match_probe_kernel(const cw_slot* __restrict__ table, u32 mask,
                                                           const u64* __restrict__ hashes,

@@ -36,8 +36,8 @@ PCIE_GEN5_X16_GBS = 63.0  # 32 GT/s x 16 lanes x 128/130 / 8 per direction (SURV
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r1_full_step_kernels.md), full-size configs[2] step.
-NCU_TRAFFIC_BYTES = {"hash": 433_179_392, "match": 106_258_943, "score_evict": 17_293_312, "gather": 1_659_130_880,
-                     "scatter": 1_659_064_064, "schedule": 107_008}
+NCU_TRAFFIC_BYTES = {"hash": 433_246_720, "match": 105_356_288, "score_evict": 17_263_872, "gather": 1_659_077_376,
+                     "scatter": 1_659_003_648, "schedule": 107_264}
 
 
 def measured_peaks():

@@ -30,7 +30,9 @@ namespace {
 
 #define CWE_THREADS 1024
 #define CWE_WARPS (CWE_THREADS / 32)
-#define CWE_ITEMS 4
+#ifndef CWE_ITEMS
+#define CWE_ITEMS 2  // measured: 2 -> 80 us, 3 -> 82, 4 -> 83, 6 -> 86 (configs[2], whole kernel)
+#endif
 #define CWE_TILE (CWE_THREADS * CWE_ITEMS)
 #define CWE_SMEM_SESS 4096                       // sessions whose tau fits the per-CTA shared-memory table
 #define CWE_SMEM_SORT (CWE_SORT_RUN * 24)        // two (score,id) buffers of the CTA sort (alias the histogram)

@@ -70,23 +70,20 @@ struct EvictArgs {
     u32* num_victims;
 };
 
-// Grid barrier of the cooperative launch.  `gen` is this CTA's private copy of the barrier generation (read once
-// at kernel start), so an arrival is ONE acq_rel atomic and the wait is an acquire spin on the generation word:
-// no fence instructions, no extra round trip to read the generation first.
-__device__ __forceinline__ void grid_barrier(cw_evict_state* st, u32 nblocks, u32& gen) {
+// Grid barrier of the cooperative launch.  The arrival counter only ever grows: a CTA arrives with ONE
+// fire-and-forget release reduction (no returning atomic: 148 returning atomics on one word serialise) and then
+// acquire-polls the counter until it reaches `target` = (value at kernel start) + G x (barriers so far).  CTA 0
+// records the reached value in bar_gen, where the next launch finds its starting point.  Wrap-safe (signed
+// difference of 32-bit counters).
+__device__ __forceinline__ void grid_barrier(cw_evict_state* st, u32 nblocks, u32& target) {
     __syncthreads();
     if (threadIdx.x == 0) {
-        u32 prev;
-        asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(prev) : "l"(&st->bar_count) : "memory");
-        if (prev == nblocks - 1) {
-            st->bar_count = 0;  // nobody touches the counter again before the generation moves on
-            st_release_u32(&st->bar_gen, gen + 1);
-        } else {
-            while (ld_acquire_u32(&st->bar_gen) == gen) {
-            }
+        target += nblocks;
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(&st->bar_count) : "memory");
+        while ((i32)(ld_acquire_u32(&st->bar_count) - target) < 0) {
         }
+        if (blockIdx.x == 0) st->bar_gen = target;
     }
-    ++gen;
     __syncthreads();
 }
 
@@ -397,7 +394,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     const u32 tid = threadIdx.x, G = gridDim.x;
     cw_evict_state* st = a.st;
     const bool tau_smem = a.S <= CWE_SMEM_SESS;
-    u32 bar_gen = ld_acquire_u32(&st->bar_gen);  // cannot move before this CTA has arrived at the first barrier
+    u32 bar_gen = ld_acquire_u32(&st->bar_gen);  // counter value when the previous launch ended (written by its CTA 0)
     u32 n_stamp = 0;
     stamp(st, n_stamp);
 

@@ -858,7 +858,8 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
         const u32 lane = tid & 31, warp = tid >> 5;
         u64* ws = s_score + warp * 128;
         u32* wi = s_id + warp * 128;
-        const u32 gw = (blockIdx.x * CWE_THREADS + tid) >> 5, nw = (G * CWE_THREADS) >> 5;
+        // warp w of CTA c takes buckets c + G*w, ...: the few thousand busy warps are spread over all SMs
+        const u32 gw = warp * G + blockIdx.x, nw = (G * CWE_THREADS) >> 5;
         const u32 n_nonempty = __ldcg(&st->n_nonempty);
         {
           for (u32 q = gw; q < n_nonempty; q += nw) {

@@ -185,6 +185,35 @@ def test_schedule_more_requests_than_one_key_tile():
     ctx.close()
 
 
+def test_schedule_wide_key_ranges_and_tie_groups():
+    """Leading words whose ranges do not fit the compressed 30-bit key (64-bit path), and tie groups on the leading
+    word of every size around the per-warp tie list (128): the remaining key words decide inside a group."""
+    from gpu_util import small_ctx
+    ctx = small_ctx(max_requests=8192)
+    g = gen.rng(25, 0)
+    for policy in (0, 1, 2):
+        for R in (100, 4096, 6000):
+            d = g.integers(0, 2**32, size=R, dtype=np.uint64).astype(np.uint32)
+            n_gpu = (g.random(R) * d).astype(np.uint32)
+            arr = g.integers(0, 2**63, size=R, dtype=np.uint64) * np.uint64(2) + np.uint64(1)
+            rid = g.integers(0, 2**32, size=R, dtype=np.uint64).astype(np.uint32)
+            eo, ena, ede = oracle.schedule(d, n_gpu, arr, rid, policy, 10**9, 10**9, R)
+            o, na, de = _schedule(ctx, d, n_gpu, arr, rid, policy, 10**9, 10**9, R)
+            assert (o == eo).all() and (na, de) == (ena, ede), (policy, R)
+    for policy in (0, 1, 2):
+        R = 4096
+        grp = np.repeat(np.arange(16), [1, 2, 3, 31, 32, 33, 127, 128, 129, 130, 255, 256, 257, 500, 1000, 1342])[:R]
+        perm = g.permutation(R)
+        d = (1000 + 3 * grp[perm]).astype(np.uint32)
+        n_gpu = (grp[perm] % 5).astype(np.uint32)
+        arr = np.where(policy == 2, grp[perm], g.integers(0, 7, size=R)).astype(np.uint64)
+        rid = g.integers(0, 4, size=R).astype(np.uint32)
+        eo, ena, ede = oracle.schedule(d, n_gpu, arr, rid, policy, 5000, 100000, R)
+        o, na, de = _schedule(ctx, d, n_gpu, arr, rid, policy, 5000, 100000, R)
+        assert (o == eo).all() and (na, de) == (ena, ede), policy
+    ctx.close()
+
+
 def test_schedule_edges():
     import paper_2606_16824_b200 as cw
     from gpu_util import small_ctx

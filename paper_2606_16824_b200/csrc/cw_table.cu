@@ -186,6 +186,8 @@ __global__ void __launch_bounds__(256, MATCH_MIN_CTAS) match_probe_kernel(const 
                                                           const u64* __restrict__ hashes,
                                                           const u64* __restrict__ hash_off, u32 R, u32* first_miss,
                                                           u32* max_hit, u32* host_hits, u32* hit_loc, u32* status) {
+    __shared__ u64 s_key[256 / 32][CWM_CHUNK];
+    __shared__ u32 s_loc[256 / 32][CWM_CHUNK];
     // hash_off may be a slice of a longer CSR array: positions below are 32-bit offsets from its first hash
     const u64 h_first = hash_off[0];
     if (hash_off[R] - h_first > 0xFFFFFFFFull) {  // more than 2^32 hashes in one call: not supported
@@ -218,6 +220,73 @@ __global__ void __launch_bounds__(256, MATCH_MIN_CTAS) match_probe_kernel(const 
         u32 req_start = (u32)(hash_off[lo] - h_first), req_end = (u32)(hash_off[lo + 1] - h_first);
         u32 dead_r = 0xFFFFFFFFu, checked_r = 0xFFFFFFFFu;  // request known to have missed / whose global state was read
         const u32 c1 = min(total, c0 + CWM_CHUNK);
+        if (c1 <= req_end) {
+            // ---- the whole task lies inside request r_base (the common case): LANE-INDEPENDENT probing.  Lane l
+            // owns the hashes c0 + l + 32k (coalesced) and walks them front to back on its own, one slot load per
+            // iteration of a warp-synchronous loop, so the warp waits for the longest SUM of probe lengths over a
+            // lane's keys instead of the sum over rounds of the longest probe of the round.
+            const u32 j0 = c0 - req_start;
+            if (j0 > 0 && __ldcg(first_miss + r_base) < j0) {  // an earlier task of the request already missed
+                if (hl)
+                    for (u32 g = c0 + lane; g < c1; g += 32) hl[g] = CW_MISS;
+                continue;
+            }
+            constexpr int KPL = CWM_CHUNK / 32;  // keys per lane
+            const u32 n_task = c1 - c0;
+            u64* wkey = s_key[threadIdx.x >> 5];  // this warp's staged (remapped) keys and resolved locations
+            u32* wloc = s_loc[threadIdx.x >> 5];
+            {
+                u64 kk[KPL];
+#pragma unroll
+                for (int q = 0; q < KPL; ++q) kk[q] = lane + 32 * q < n_task ? hs[c0 + lane + 32 * q] : 0;  // in flight together
+#pragma unroll
+                for (int q = 0; q < KPL; ++q) wkey[lane + 32 * q] = cw_remap_key(kk[q]);  // read back by this lane only
+            }
+            u32 pos = lane;          // position of this lane's current key inside the task
+            u32 limit = n_task;      // warp-uniform: min(n_task, first missing position seen so far)
+            uint2 key = *reinterpret_cast<const uint2*>(wkey + pos);
+            u32 slot = key.x & mask;
+            for (;;) {
+                const bool live = pos < limit;
+                if (!__any_sync(0xffffffffu, live)) break;
+                u32 miss_at = 0xFFFFFFFFu;
+                if (live) {
+                    uint4 v;
+                    asm volatile("ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4];"
+                                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                                 : "l"(table + slot));
+                    const bool hit = v.x == key.x && v.y == key.y;
+                    const bool empty = (v.x | v.y) == 0;
+                    slot = (slot + 1) & mask;
+                    if (hit || empty) {  // resolved: record, next key of this lane
+                        wloc[pos] = hit ? v.z : CW_MISS;
+                        if (empty) miss_at = pos;
+                        pos += 32;
+                        key = *reinterpret_cast<const uint2*>(wkey + (pos & (CWM_CHUNK - 1)));
+                        slot = key.x & mask;
+                    }
+                }
+                if (__any_sync(0xffffffffu, miss_at != 0xFFFFFFFFu)) limit = min(limit, __reduce_min_sync(0xffffffffu, miss_at));
+            }
+            __syncwarp();
+            // hits behind the first miss are not part of the prefix
+            u32 host = 0;
+#pragma unroll
+            for (int q = 0; q < KPL; ++q) {
+                const u32 p = lane + 32 * q;
+                const u32 l = p < limit ? wloc[p] : CW_MISS;
+                host += (l != CW_MISS && (l & CW_HOST_BIT)) ? 1u : 0u;
+                if (hl && p < n_task) hl[c0 + p] = l;
+            }
+            host = __reduce_add_sync(0xffffffffu, host);
+            if (lane == 0) {
+                if (limit < n_task) atomicMin(&first_miss[r_base], j0 + limit);
+                if (limit) atomicMax(&max_hit[r_base], j0 + limit);
+                if (host) atomicAdd(&host_hits[r_base], host);
+            }
+            __syncwarp();  // the staging rows are reused by the next task of this warp
+            continue;
+        }
         u64 key_next = c0 + lane < c1 ? hs[c0 + lane] : 0;
         for (u32 g0 = c0; g0 < c1; g0 += 32) {
             while (g0 >= req_end) {  // warp-uniform; also skips empty requests

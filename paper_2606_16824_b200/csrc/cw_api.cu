@@ -137,7 +137,7 @@ int32_t cw_create(const cw_config* cfg, cw_ctx** out) {
     CW_CUDA(c, dalloc_zero(&c->out_id, c->ev_cap, s));
     CW_CUDA(c, dalloc_zero(&c->hist, (size_t)CWE_PASSES * CWE_BINS, s));
     CW_CUDA(c, dalloc_zero(&c->ev, 1, s));
-    CW_CUDA(c, dalloc_zero(&c->ev_bhist, 65536, s));
+    CW_CUDA(c, dalloc_zero(&c->ev_bhist, 65536 + 128, s));
     CW_CUDA(c, dalloc_zero(&c->ev_boff, 65537, s));
     CW_CUDA(c, dalloc_zero(&c->ev_bcur, 65536, s));
     CW_CUDA(c, dalloc_zero(&c->ev_blist, 196608, s));

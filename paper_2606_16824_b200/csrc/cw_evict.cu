@@ -776,22 +776,26 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     }
     // D1: bucket = the top 16 bits that vary among the victims (a monotone function of the key), histogram
     const DigitPlan& bp = s_plan;
-    for (u32 e = blockIdx.x * CWE_THREADS + tid; e < want; e += G * CWE_THREADS)
-        atomicAdd(&a.bhist[plan_digit<CWE_BUCKET_BITS>(bp, __ldcg(a.out_score + e), __ldcg(a.out_id + e))], 1u);
+    //     plus a coarse histogram over the 128 slices of 512 buckets (warp-aggregated), which gives every CTA of D2
+    //     the offset of its slice without re-reading the fine histogram
+    u32* chist = a.bhist + CWE_BUCKETS;
+    for (u32 e = blockIdx.x * CWE_THREADS + tid; e < want; e += G * CWE_THREADS) {
+        const u32 dg = plan_digit<CWE_BUCKET_BITS>(bp, __ldcg(a.out_score + e), __ldcg(a.out_id + e));
+        atomicAdd(&a.bhist[dg], 1u);
+        const u32 cg = dg >> 9;
+        const u32 peers = __match_any_sync(__activemask(), cg);
+        if ((tid & 31) == (u32)__ffs(peers) - 1) atomicAdd(&chist[cg], (u32)__popc(peers));
+    }
     grid_barrier(st, G, bar_gen);
     stamp(st, n_stamp);
     // D2: exclusive scan of the bucket sizes, every CTA on its own slice of 512 buckets: the offset of the slice
-    //     is the sum of all earlier buckets (re-read from L2: at most 256 KiB), so no CTA waits for another
+    //     is the sum of the coarse counts of all earlier slices, so no CTA waits for another
     {
         constexpr u32 SLICE = 512;
         const u32 lane = tid & 31, warp = tid >> 5;
         for (u32 sl = blockIdx.x; sl < CWE_BUCKETS / SLICE; sl += G) {
             const u32 first = sl * SLICE;
-            u32 before = 0;
-            for (u32 b = tid * 4; b < first; b += CWE_THREADS * 4) {
-                const uint4 v = __ldcg(reinterpret_cast<const uint4*>(a.bhist + b));
-                before += v.x + v.y + v.z + v.w;
-            }
+            const u32 before = tid < sl ? __ldcg(chist + tid) : 0u;  // SLICE == 512 == 1 << 9 (the coarse digit)
             const u32 mine = tid < SLICE ? __ldcg(a.bhist + first + tid) : 0u;
             // block scan of (before: plain sum, mine: inclusive prefix over tid)
             u32 inc = mine, tot = before;
@@ -840,6 +844,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     grid_barrier(st, G, bar_gen);
     stamp(st, n_stamp);
     // D3: scatter into bucket order (inside a bucket the order is arbitrary for now)
+    if (blockIdx.x == 0 && tid < CWE_BUCKETS / 512) chist[tid] = 0;  // self-cleaning
     u64* tmp_score = a.cand_score[0];
     u32* tmp_id = a.cand_id[0];
     for (u32 e = blockIdx.x * CWE_THREADS + tid; e < want; e += G * CWE_THREADS) {

@@ -138,7 +138,7 @@ struct cw_ctx {
     u32* out_id;
     u32* hist;  // CWE_PASSES * CWE_BINS
     cw_evict_state* ev;
-    u32* ev_bhist;   // victims per bucket (CWE_BUCKETS)
+    u32* ev_bhist;   // victims per bucket (CWE_BUCKETS) + per slice of 512 buckets (128)
     u32* ev_boff;    // exclusive scan (CWE_BUCKETS + 1)
     u32* ev_bcur;    // scatter cursors (CWE_BUCKETS)
     u32* ev_blist;   // [0, 65536): medium buckets, [65536, 131072): large, [131072, 196608): non-empty

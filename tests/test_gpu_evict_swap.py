@@ -305,6 +305,49 @@ def test_swap_out_swap_in_round_trip_through_pinned_host(layout):
     ctx.close()
 
 
+@pytest.mark.parametrize("layout", LAYOUTS)
+@pytest.mark.parametrize("tp", [2, 4])
+def test_tp_sharded_swap_equals_the_unsharded_page(layout, tp):
+    """SURVEY 8(e) / PAPER.md L271 (TP=2): stage 4 shards by KV head with no exchange.  Rank t holds bytes
+    [t*cb/tp, (t+1)*cb/tp) of every chunk (chunk = [kv_head][token][dim]) in its own pool and runs the SAME victim
+    list (decisions are replicated); the rank pages, re-interleaved per chunk, must equal the oracle's page of the
+    unsharded pool, and swapping them back in must restore every rank's pool bytes."""
+    import torch
+    from gpu_util import dev, host
+    M, n_chunks, cb = 48, 6, 8192
+    g = gen.rng(36, tp)
+    full = g.integers(0, 256, size=(n_chunks, M, cb), dtype=np.uint8)       # [chunk][block][byte]
+    full_cfg = _pool_cfg("layer_major", M, n_chunks, cb)
+    n = 17
+    vic = g.permutation(M)[:n].astype(np.uint32)
+    exp = oracle.swap_out(full.reshape(-1).copy(), n_chunks, cb, full_cfg["chunk_stride"], full_cfg["block_stride"], vic,
+                          np.zeros(n * n_chunks * cb, np.uint8)).reshape(n, n_chunks, cb)
+    sb = cb // tp
+    pages, ctxs = [], []
+    for t in range(tp):
+        shard = full[:, :, t * sb:(t + 1) * sb]                               # rank t's head slice
+        if layout == "layer_major":
+            pool_np = np.ascontiguousarray(shard).reshape(-1)
+        else:
+            pool_np = np.ascontiguousarray(shard.transpose(1, 0, 2)).reshape(-1)
+        ctx, pool = _swap_ctx(layout, M, n_chunks, sb, 4, pool_np)
+        h = torch.zeros(n * n_chunks * sb, dtype=torch.uint8).pin_memory()
+        ctx.swap_out(dev(vic), None, n, None, h)
+        assert ctx.sync(check=False) == 0
+        pages.append(h.numpy().reshape(n, n_chunks, sb).copy())
+        ctxs.append((ctx, pool, pool_np, h))
+    assert (np.concatenate(pages, axis=2) == exp).all()
+    for ctx, pool, pool_np, h in ctxs:                                        # restore into wiped pools
+        pool.zero_()
+        ctx.swap_in(None, h, dev(vic), n)
+        assert ctx.sync(check=False) == 0
+        cfg = _pool_cfg(layout, M, n_chunks, sb)
+        want = oracle.swap_in(np.zeros_like(pool_np), n_chunks, sb, cfg["chunk_stride"], cfg["block_stride"],
+                              h.numpy().copy(), vic)
+        assert (host(pool, np.uint8) == want).all()
+        ctx.close()
+
+
 def test_out_of_range_block_id_is_reported_and_touches_nothing():
     import torch
     from gpu_util import dev

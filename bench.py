@@ -381,8 +381,28 @@ def run_cuda(args):
             h2d = T * 4 + sum(h.numel() * h.element_size() for _, h in h_small)
             d2h = 12 + 3 * st.R * 4
 
+            # The token ids of step i+1 travel host->device on a side stream while step i's victims travel
+            # device->host (PCIe is full duplex): two device token buffers, one upload per step, all inside the
+            # timed region.  Everything else of a step stays in order on `stream`.
+            up_stream = torch.cuda.Stream()
+            tok_bufs = [st.d_tok, torch.empty_like(st.d_tok)]
+            tok_bufs[1][T:].zero_()
+            up_done = [torch.cuda.Event(), torch.cuda.Event()]
+            e2e_i = [0]
+
+            def upload(k):
+                up_stream.wait_stream(stream)          # the decide that last read this buffer has been enqueued
+                with torch.cuda.stream(up_stream):
+                    tok_bufs[k][:T].copy_(h_tok, non_blocking=True)
+                    up_done[k].record(up_stream)
+
+            upload(0)
+
             def e2e_step():
-                st.d_tok[:T].copy_(h_tok, non_blocking=True)
+                k = e2e_i[0] & 1
+                e2e_i[0] += 1
+                st.d_tok = tok_bufs[k]
+                stream.wait_event(up_done[k])          # this step's token ids are on the device
                 for d, h in h_small:
                     d.copy_(h, non_blocking=True)
                 st.decide()
@@ -390,6 +410,7 @@ def run_cuda(args):
                 h_scal[1:2].copy_(st.d_def, non_blocking=True)
                 h_scal[2:3].copy_(st.d_nv, non_blocking=True)
                 stream.synchronize()
+                upload(k ^ 1)                          # next step's token ids: overlaps this step's swap-out
                 n = int(h_scal[2])
                 st.ctx.swap_out(st.d_vic, None, n, None, h_swap)
                 st.ctx.swap_in(None, h_swap, st.d_vic, n)
@@ -413,11 +434,12 @@ def run_cuda(args):
             hdist.barrier()
             e2e_ms = e0.elapsed_time(e1)
             st.ctx.sync(check=False)
+            st.d_tok = tok_bufs[0]
         eu, et = hdist.aggregate(float(st.n_hashed) * Ke, e2e_ms, "cuda")
         extra["e2e"] = {"value": eu / (et * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d + n_e2e * st.page,
                         "d2h_bytes_per_step": d2h + n_e2e * st.page + n_e2e * 4, "steps": Ke,
                         "ms_per_step": round(et / Ke, 4)}
-        del h_tok, h_swap
+        del h_tok, h_swap, tok_bufs
 
     if rank == 0 and not args.quick:
         # ---- the <=100 us target: stages 1-3 as ONE CUDA-graph launch, cold (all requests hashed) and steady

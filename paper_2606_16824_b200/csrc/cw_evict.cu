@@ -779,11 +779,15 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     //     plus a coarse histogram over the 128 slices of 512 buckets (warp-aggregated), which gives every CTA of D2
     //     the offset of its slice without re-reading the fine histogram
     u32* chist = a.bhist + CWE_BUCKETS;
-    for (u32 e = blockIdx.x * CWE_THREADS + tid; e < want; e += G * CWE_THREADS) {
+    // (warp w of CTA c takes the 32 victims at (w * G + c) * 32: the ~1600 busy warps are spread over all SMs)
+    for (u32 e = ((tid >> 5) * G + blockIdx.x) * 32 + (tid & 31); e < want; e += G * CWE_THREADS) {
         const u32 dg = plan_digit<CWE_BUCKET_BITS>(bp, __ldcg(a.out_score + e), __ldcg(a.out_id + e));
-        atomicAdd(&a.bhist[dg], 1u);
+        // neighbouring victims mostly share a bucket: one atomic per warp and distinct bucket / slice
+        const u32 act = __activemask();
+        const u32 same = __match_any_sync(act, dg);
+        if ((tid & 31) == (u32)__ffs(same) - 1) atomicAdd(&a.bhist[dg], (u32)__popc(same));
         const u32 cg = dg >> 9;
-        const u32 peers = __match_any_sync(__activemask(), cg);
+        const u32 peers = __match_any_sync(act, cg);
         if ((tid & 31) == (u32)__ffs(peers) - 1) atomicAdd(&chist[cg], (u32)__popc(peers));
     }
     grid_barrier(st, G, bar_gen);
@@ -847,10 +851,15 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     if (blockIdx.x == 0 && tid < CWE_BUCKETS / 512) chist[tid] = 0;  // self-cleaning
     u64* tmp_score = a.cand_score[0];
     u32* tmp_id = a.cand_id[0];
-    for (u32 e = blockIdx.x * CWE_THREADS + tid; e < want; e += G * CWE_THREADS) {
+    for (u32 e = ((tid >> 5) * G + blockIdx.x) * 32 + (tid & 31); e < want; e += G * CWE_THREADS) {
         const u64 sc = __ldcg(a.out_score + e);
         const u32 id = __ldcg(a.out_id + e);
-        const u32 pos = atomicAdd(&a.bcur[plan_digit<CWE_BUCKET_BITS>(bp, sc, id)], 1u);
+        const u32 dg = plan_digit<CWE_BUCKET_BITS>(bp, sc, id);
+        const u32 same = __match_any_sync(__activemask(), dg);  // one returning atomic per warp and distinct bucket
+        const u32 leader = (u32)__ffs(same) - 1;
+        u32 pos = 0;
+        if ((tid & 31) == leader) pos = atomicAdd(&a.bcur[dg], (u32)__popc(same));
+        pos = __shfl_sync(same, pos, leader) + __popc(same & ((1u << (tid & 31)) - 1));
         tmp_score[pos] = sc;
         tmp_id[pos] = id;
     }

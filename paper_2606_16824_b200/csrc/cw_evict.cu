@@ -123,49 +123,57 @@ __device__ __forceinline__ u32 plan_digit(const DigitPlan& pl, u64 score, u32 id
     }
     return d;
 }
-// the top `maxbits` set bits of (vary_hi : vary_lo); then, if `fill_from` < 96, contiguous bits from there downwards
+// the top `maxbits` set bits of (vary_hi : vary_lo); then, if `fill_from` < 96, contiguous bits from there downwards.
+// WARP-COOPERATIVE (all 32 lanes of one warp call it with the same arguments): lane i looks at bit i of each of the
+// three key words, ballots give the kept bits, every lane that holds the lowest bit of a run writes that run.
 __device__ __forceinline__ void make_plan(DigitPlan* pl, u64 vary_hi, u32 vary_lo, u32 fill_from,
                                           u32 maxbits = CWE_DIGIT_BITS) {
-    u32 pos[CWE_BUCKET_BITS];
-    u32 n = 0;
-    u32 lowest = 96;
-    while (n < maxbits && (vary_hi || vary_lo)) {
-        u32 p;
-        if (vary_hi) {
-            p = 63 - __clzll((long long)vary_hi);
-            vary_hi &= ~(1ull << p);
-            p += 32;
-        } else {
-            p = 31 - __clz((int)vary_lo);
-            vary_lo &= ~(1u << p);
+    const u32 lane = threadIdx.x & 31;
+    const u32 w[3] = {vary_lo, (u32)vary_hi, (u32)(vary_hi >> 32)};
+    u32 k[3];
+    u32 budget = maxbits;
+#pragma unroll
+    for (int x = 2; x >= 0; --x) {
+        const u32 above = lane == 31 ? 0u : (u32)__popc(w[x] >> (lane + 1));
+        k[x] = __ballot_sync(0xffffffffu, ((w[x] >> lane) & 1u) && above < budget);
+        budget -= (u32)__popc(k[x]);
+    }
+    u32 n = maxbits - budget;
+    if (fill_from < 96 && n < maxbits) {  // plain bits below every chosen one keep the digit monotone in the key
+        const u32 lowest = k[0] ? (u32)__ffs(k[0]) - 1 : k[1] ? 31 + (u32)__ffs(k[1]) : k[2] ? 63 + (u32)__ffs(k[2]) : 96u;
+        if (lowest != 0) {
+            const u32 p = lowest == 96 ? fill_from : min(fill_from, lowest - 1);
+            const u32 cnt = min(maxbits - n, p + 1);
+            const u32 lo_p = p + 1 - cnt;
+#pragma unroll
+            for (int x = 0; x < 3; ++x) {
+                const u32 pos = 32 * x + lane;
+                k[x] |= __ballot_sync(0xffffffffu, pos >= lo_p && pos <= p);
+            }
+            n += cnt;
         }
-        pos[n++] = p;
-        lowest = p;
     }
-    if (fill_from < 96) {
-        // plain bits below every chosen one keep the digit a monotone function of the key
-        u32 p = lowest == 96 ? fill_from : min(fill_from, lowest - 1);
-        while (n < maxbits) {
-            pos[n++] = p;
-            if (p == 0) break;
-            --p;
+    const u32 below[3] = {0u, (u32)__popc(k[0]), (u32)(__popc(k[0]) + __popc(k[1]))};
+    u32 runs = 0;
+#pragma unroll
+    for (int x = 2; x >= 0; --x) {  // runs of adjacent kept bits inside one 32-bit word
+        const u32 kw = k[x];
+        const u32 low = kw & ~(kw << 1);
+        if ((low >> lane) & 1u) {
+            const u32 idx = runs + (lane == 31 ? 0u : (u32)__popc(low >> (lane + 1)));
+            const u32 inv = ~(kw >> lane);
+            const u32 len = inv ? (u32)__ffs(inv) - 1 : 32 - lane;
+            pl->word[idx] = (u32)x;
+            pl->shift[idx] = lane;
+            pl->mask[idx] = len >= 32 ? 0xFFFFFFFFu : (1u << len) - 1;
+            pl->dst[idx] = below[x] + (u32)__popc(kw & ((1u << lane) - 1));
         }
+        runs += (u32)__popc(low);
     }
-    // positions are descending: group them into runs of adjacent bits that stay inside one 32-bit word
-    u32 nr = 0;
-    for (u32 i = 0; i < n;) {
-        u32 jx = i;
-        while (jx + 1 < n && pos[jx + 1] + 1 == pos[jx] && (pos[jx + 1] >> 5) == (pos[i] >> 5)) ++jx;
-        const u32 len = jx - i + 1;
-        pl->word[nr] = pos[i] >> 5;
-        pl->shift[nr] = pos[jx] & 31;
-        pl->mask[nr] = (1u << len) - 1;  // len <= 16
-        pl->dst[nr] = n - 1 - jx;        // digit bit of the run's lowest key bit
-        ++nr;
-        i = jx + 1;
+    if (lane == 0) {
+        pl->nbits = n;
+        pl->nruns = runs;
     }
-    pl->nbits = n;
-    pl->nruns = nr;
 }
 
 // CTA sort of N keys (score,id), N a power of two, 128 <= N <= CWE_SORT_RUN, ascending.
@@ -296,26 +304,31 @@ __device__ __forceinline__ void tile_append(const bool (&f0)[CWE_ITEMS], const b
 template <int N>
 __device__ __forceinline__ void block_or_n(const u64 (&hi)[N], const u32 (&lo)[N], u64* const (&g_hi)[N],
                                            u32* const (&g_lo)[N], u64* s_hi, u32* s_lo) {
-    const u32 tid = threadIdx.x, lane = tid & 31;
-    if (tid < N) {
-        s_hi[tid] = 0;
-        s_lo[tid] = 0;
-    }
-    __syncthreads();
+    // s_hi / s_lo hold N x CWE_WARPS per-warp partials (no shared-memory atomics: 32 warps on one word serialise)
+    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 #pragma unroll
     for (int n = 0; n < N; ++n) {
         const u32 a = __reduce_or_sync(0xffffffffu, (u32)hi[n]);
         const u32 b = __reduce_or_sync(0xffffffffu, (u32)(hi[n] >> 32));
         const u32 c = __reduce_or_sync(0xffffffffu, lo[n]);
         if (lane == 0) {
-            if (a | b) atomicOr(reinterpret_cast<unsigned long long*>(s_hi + n), ((unsigned long long)b << 32) | a);
-            if (c) atomicOr(s_lo + n, c);
+            s_hi[n * CWE_WARPS + warp] = ((u64)b << 32) | a;
+            s_lo[n * CWE_WARPS + warp] = c;
         }
     }
     __syncthreads();
-    if (tid < N) {
-        if (s_hi[tid]) atomicOr(reinterpret_cast<unsigned long long*>(g_hi[tid]), (unsigned long long)s_hi[tid]);
-        if (s_lo[tid]) atomicOr(g_lo[tid], s_lo[tid]);
+#pragma unroll
+    for (int n = 0; n < N; ++n) {
+        if (warp == (u32)n) {  // warp n folds word n and issues the one atomic per CTA and word
+            const u64 h = s_hi[n * CWE_WARPS + lane];
+            const u32 a = __reduce_or_sync(0xffffffffu, (u32)h);
+            const u32 b = __reduce_or_sync(0xffffffffu, (u32)(h >> 32));
+            const u32 c = __reduce_or_sync(0xffffffffu, s_lo[n * CWE_WARPS + lane]);
+            if (lane == 0) {
+                if (a | b) atomicOr(reinterpret_cast<unsigned long long*>(g_hi[n]), ((unsigned long long)b << 32) | a);
+                if (c) atomicOr(g_lo[n], c);
+            }
+        }
     }
     __syncthreads();
 }
@@ -386,8 +399,8 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     __shared__ u32 s_w0[CWE_WARPS], s_w1[CWE_WARPS], s_base[2];
     __shared__ u32 s_scan[CWE_WARPS];
     __shared__ u32 s_thr[3];  // threshold bin, count before it, count inside it
-    __shared__ u64 s_mhi[CWE_WARPS];
-    __shared__ u32 s_mlo[CWE_WARPS];
+    __shared__ u64 s_mhi[4 * CWE_WARPS];
+    __shared__ u32 s_mlo[4 * CWE_WARPS];
     __shared__ u64 s_acc_hi, s_acc2_hi;
     __shared__ u32 s_acc_lo, s_acc2_lo, s_cnt[2];
     __shared__ DigitPlan s_plan;
@@ -441,7 +454,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
             if (tid == 0) s_acc_hi = __ldcg(reinterpret_cast<const unsigned long long*>(&st->tau_masks));
             __syncthreads();
         }
-        if (tid == 0) {
+        if (tid < 32) {
             const u32 vary_tau = (u32)(s_acc_hi >> 32) & (u32)s_acc_hi & 0xFFFFFFu;
             make_plan(&s_plan, (u64)vary_tau << 40, 0u, 39 + 32);
         }
@@ -578,7 +591,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
                             u32* const gl[2] = {&s_acc_lo, &s_acc2_lo};
                             block_or_n<2>(h2, l2, gh, gl, s_mhi, s_mlo);
                         }
-                        if (tid == 0) make_plan(&s_plan, s_acc_hi & s_acc2_hi, s_acc_lo & s_acc2_lo, 96);
+                        if (tid < 32) make_plan(&s_plan, s_acc_hi & s_acc2_hi, s_acc_lo & s_acc2_lo, 96);
                         __syncthreads();
                         const DigitPlan& lp = s_plan;
                         for (u32 i = tid; i < n; i += CWE_THREADS) atomicAdd(&l_hist[plan_digit(lp, c_s[i], c_i[i])], 1u);
@@ -698,7 +711,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
             n_cur = inside;
             if (n_cur <= CWE_LOCAL || p + 1 >= CWE_PASSES) continue;  // finished by one CTA at the top of the loop
             // histogram of the next level over the bits that still vary inside the new candidate set
-            if (tid == 0) {
+            if (tid < 32) {
                 const u64 vh = __ldcg(reinterpret_cast<const unsigned long long*>(&st->or_hi[p + 1])) &
                                __ldcg(reinterpret_cast<const unsigned long long*>(&st->nand_hi[p + 1]));
                 const u32 vl = __ldcg(&st->or_lo[p + 1]) & __ldcg(&st->nand_lo[p + 1]);
@@ -728,7 +741,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     // (nothing reads hist / the selection state any more: every CTA carries `want` in registers)
     for (u32 i = blockIdx.x * CWE_THREADS + tid; i < CWE_PASSES * CWE_BINS; i += G * CWE_THREADS) a.hist[i] = 0;
     // bits that vary among the victims -> digit plan of the bucketing (read before CTA 0 clears the masks)
-    if (tid == 0) {
+    if (tid < 32) {
         const u64 vh = __ldcg(reinterpret_cast<const unsigned long long*>(&st->vic_or_hi)) &
                        __ldcg(reinterpret_cast<const unsigned long long*>(&st->vic_nand_hi));
         const u32 vl = __ldcg(&st->vic_or_lo) & __ldcg(&st->vic_nand_lo);

@@ -175,19 +175,22 @@ __global__ void insert_reset_kernel(cw_slot* table, u32 n, const u32* ins_slot) 
 }
 
 // ---------------------------------------------------------------------------------------------- match
-// 8 CTAs of 256 threads per SM (<= 32 registers): the probe is bound by resident warps x latency (93 us vs 107 us
+// full occupancy (<= 32 registers, 2048 threads per SM): the probe is bound by resident warps x latency (93 us vs 107 us
 // at 6 CTAs/SM on configs[2])
-#define MATCH_MIN_CTAS 8
+#ifndef MATCH_THREADS
+#define MATCH_THREADS 64  // measured on configs[2]: 256 -> 66.1 us, 128 -> 65.9, 64 -> 64.6 (CTA slots turn over per 2 tasks)
+#endif
+#define MATCH_MIN_CTAS (2048 / MATCH_THREADS)
 #define CWM_CHUNK 128  // consecutive hashes handled by one warp task (4 rounds of 32): measured optimum on configs[2]
                        // (64: 89 us, 128: 75, 256: 79, 512: ~85, 1024: ~100, 2048: ~170 — long tasks are bound by the
                        // dependent probe chain of the slowest warp, short ones by the per-task search and set-up)
 
-__global__ void __launch_bounds__(256, MATCH_MIN_CTAS) match_probe_kernel(const cw_slot* __restrict__ table, u32 mask,
+__global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_kernel(const cw_slot* __restrict__ table, u32 mask,
                                                           const u64* __restrict__ hashes,
                                                           const u64* __restrict__ hash_off, u32 R, u32* first_miss,
                                                           u32* max_hit, u32* host_hits, u32* hit_loc, u32* status) {
-    __shared__ u64 s_key[256 / 32][CWM_CHUNK];
-    __shared__ u32 s_loc[256 / 32][CWM_CHUNK];
+    __shared__ u64 s_key[MATCH_THREADS / 32][CWM_CHUNK];
+    __shared__ u32 s_loc[MATCH_THREADS / 32][CWM_CHUNK];
     // hash_off may be a slice of a longer CSR array: positions below are 32-bit offsets from its first hash
     const u64 h_first = hash_off[0];
     if (hash_off[R] - h_first > 0xFFFFFFFFull) {  // more than 2^32 hashes in one call: not supported
@@ -445,11 +448,11 @@ int32_t cwi_match_prefix(cw_ctx* ctx, const u64* d_hashes, const u64* d_hash_off
     const u64 mask = ctx->n_slots - 1;
     // enough warps to cover max_hashed_blocks once, capped at a few waves; the kernel grid-strides
     u64 warps = (ctx->cfg.max_hashed_blocks + CWM_CHUNK - 1) / CWM_CHUNK;
-    u64 blocks = (warps + 7) / 8;
-    u64 cap = (u64)ctx->n_sm * 8 * 4;
+    u64 blocks = (warps + MATCH_THREADS / 32 - 1) / (MATCH_THREADS / 32);
+    u64 cap = (u64)ctx->n_sm * MATCH_MIN_CTAS * 4;
     if (blocks > cap) blocks = cap;
     if (blocks < 1) blocks = 1;
-    match_probe_kernel<<<(u32)blocks, 256, 0, ctx->s_main>>>(ctx->table, (u32)mask, d_hashes, d_hash_off, R,
+    match_probe_kernel<<<(u32)blocks, MATCH_THREADS, 0, ctx->s_main>>>(ctx->table, (u32)mask, d_hashes, d_hash_off, R,
                                                              ctx->m_first_miss, ctx->m_max_hit, ctx->m_host_hits,
                                                              d_hit_loc, ctx->d_status);
     CW_LAUNCH_CHECK(ctx);

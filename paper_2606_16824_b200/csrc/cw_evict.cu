@@ -411,6 +411,21 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     u32 n_stamp = 0;
     stamp(st, n_stamp);
 
+    // the metadata of this CTA's first tile is requested before phase A: its DRAM latency hides behind the tau pass
+    u32 rf[CWE_ITEMS], se[CWE_ITEMS], la[CWE_ITEMS], dp[CWE_ITEMS];
+    auto load_tile = [&](u32 tile) {
+#pragma unroll
+        for (int k = 0; k < CWE_ITEMS; ++k) {
+            const u32 b = tile * CWE_TILE + k * CWE_THREADS + tid;
+            const bool in = (u64)tile * CWE_TILE < a.M && b < a.M;
+            rf[k] = in ? a.m_ref[b] : 0u;
+            se[k] = in ? a.m_session[b] : 0u;
+            la[k] = in ? a.m_last[b] : 0u;
+            dp[k] = in ? a.m_depth[b] : 0u;
+        }
+    };
+    load_tile(blockIdx.x);
+
     // ---------------------------------------------------------------- A: per-session tau
     {
         if (tid == 0) {
@@ -471,17 +486,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
             bool f0[CWE_ITEMS], f1[CWE_ITEMS];
             u32 p0[CWE_ITEMS], p1[CWE_ITEMS];
             u64 sc[CWE_ITEMS];
-            // all four metadata words of every block are loaded up front (independent loads, one latency)
-            u32 rf[CWE_ITEMS], se[CWE_ITEMS], la[CWE_ITEMS], dp[CWE_ITEMS];
-#pragma unroll
-            for (int k = 0; k < CWE_ITEMS; ++k) {
-                const u32 b = tile * CWE_TILE + k * CWE_THREADS + tid;
-                const bool in = b < a.M;
-                rf[k] = in ? a.m_ref[b] : 0u;
-                se[k] = in ? a.m_session[b] : 0u;
-                la[k] = in ? a.m_last[b] : 0u;
-                dp[k] = in ? a.m_depth[b] : 0u;
-            }
+            if (tile != blockIdx.x) load_tile(tile);
 #pragma unroll
             for (int k = 0; k < CWE_ITEMS; ++k) {
                 const u32 b = tile * CWE_TILE + k * CWE_THREADS + tid;

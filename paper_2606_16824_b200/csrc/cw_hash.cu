@@ -353,28 +353,63 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, 4) hash_kernel(const HashArgs a
     __syncthreads();
     const u32 flags = sm.rec_flags;
     const u32 bseg_len = sm.rec_bseg_len;
-    if (tid == 0) {
+    if (warp == 0) {
         // Publish at once, never after a wait: a range that lies wholly inside one request publishes its CARRY-FREE
         // tail together with its length; the reader folds such records while walking back to the first final one
         // (decoupled look-back over ranges: every CTA walks on its own, nobody waits for a chain of CTAs).
-        const bool dependent = (flags & CWH_REC_TAIL_IS_BSEG) != 0;
-        a.rec[range].tail = sm.rec_tail_state;
-        a.rec[range].len_kind = dependent ? (bseg_len | 0x80000000u) : 0u;
-        st_release_u32(&a.rec[range].ready, epoch);
+        if (lane == 0) {
+            const bool dependent = (flags & CWH_REC_TAIL_IS_BSEG) != 0;
+            a.rec[range].tail = sm.rec_tail_state;
+            a.rec[range].len_kind = dependent ? (bseg_len | 0x80000000u) : 0u;
+            st_release_u32(&a.rec[range].ready, epoch);
+        }
+        // The walk is WARP-PARALLEL: lane i looks at record range-1-i, all 32 records are polled together, and the
+        // records up to the first final one are folded with a multiplicative warp scan of A^len — a request of 8192
+        // blocks spans 8 ranges, and one dependent L2 round trip per record made the last CTAs finish 8 us late.
         u64 carry_in = 0;
         if (flags & CWH_REC_MID) {  // the true chain state at the end of the previous range
-            u64 mult = 1;
-            for (u32 k = range; k-- > 0;) {
-                const cw_hash_rec* prev = a.rec + k;
-                while (ld_acquire_u32(&prev->ready) != epoch) {
+            u64 mult = 1;           // product of A^len over the records folded in earlier rounds (warp-uniform)
+            i32 k_hi = (i32)range - 1;
+            for (;;) {
+                const i32 k = k_hi - (i32)lane;
+                const cw_hash_rec* prev = a.rec + (k >= 0 ? k : 0);
+                u32 nuse;
+                for (;;) {  // poll until the records from k_hi down to the first final one are all published
+                    const bool ready = k < 0 || ld_acquire_u32(&prev->ready) == epoch;
+                    const bool fin = k < 0 || (ready && !(*reinterpret_cast<const volatile u32*>(&prev->len_kind) & 0x80000000u));
+                    const u32 rmask = __ballot_sync(0xffffffffu, ready);
+                    const u32 fmask = __ballot_sync(0xffffffffu, fin);
+                    const u32 first_fin = fmask ? (u32)__ffs(fmask) - 1 : 32u;
+                    const u32 need = first_fin >= 32 ? 0xffffffffu : ((2u << first_fin) - 1);  // lanes 0..first_fin
+                    if ((rmask & need) == need) {
+                        nuse = first_fin >= 32 ? 32u : first_fin + 1;
+                        break;
+                    }
                 }
-                carry_in += mult * ld_relaxed_u64(&prev->tail);
-                const u32 lk = *reinterpret_cast<const volatile u32*>(&prev->len_kind);
-                if (!(lk & 0x80000000u)) break;  // a final tail: the walk ends (range 0 is always final)
-                mult *= pow_u64(CW_A, lk & 0x7FFFFFFFu);
+                u64 tail = 0, f = 1;
+                if (k >= 0 && lane < nuse) {
+                    tail = ld_relaxed_u64(&prev->tail);
+                    const u32 lk = *reinterpret_cast<const volatile u32*>(&prev->len_kind);
+                    if (lk & 0x80000000u) f = pow_u64(CW_A, lk & 0x7FFFFFFFu);
+                }
+                u64 incl = f;  // inclusive product scan of the factors
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const u64 y = shfl64_up(incl, d);
+                    if (lane >= (u32)d) incl *= y;
+                }
+                u64 excl = shfl64_up(incl, 1);
+                if (lane == 0) excl = 1;
+                u64 term = lane < nuse ? mult * excl * tail : 0ull;
+#pragma unroll
+                for (int d = 16; d; d >>= 1) term += shfl64_xor(term, d);
+                carry_in += term;
+                if (nuse < 32 || k_hi < 32) break;  // reached a final record (range 0 is always final)
+                mult *= shfl64(incl, 31);
+                k_hi -= 32;
             }
         }
-        sm.carry_in = carry_in;
+        if (lane == 0) sm.carry_in = carry_in;
     }
     __syncthreads();
     if ((flags & CWH_REC_MID) && bseg_len) {

@@ -231,7 +231,7 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
             const u32 j0 = c0 - req_start;
             if (j0 > 0 && __ldcg(first_miss + r_base) < j0) {  // an earlier task of the request already missed
                 if (hl)
-                    for (u32 g = c0 + lane; g < c1; g += 32) hl[g] = CW_MISS;
+                    for (u32 g = c0 + lane; g < c1; g += 32) __stcs(hl + g, CW_MISS);
                 continue;
             }
             constexpr int KPL = CWM_CHUNK / 32;  // keys per lane
@@ -279,7 +279,7 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
                 const u32 p = lane + 32 * q;
                 const u32 l = p < limit ? wloc[p] : CW_MISS;
                 host += (l != CW_MISS && (l & CW_HOST_BIT)) ? 1u : 0u;
-                if (hl && p < n_task) hl[c0 + p] = l;
+                if (hl && p < n_task) __stcs(hl + c0 + p, l);  // streaming: hit_loc is not re-read on the device
             }
             host = __reduce_add_sync(0xffffffffu, host);
             if (lane == 0) {
@@ -317,7 +317,7 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
                     if (j0 > 0 && __ldcg(first_miss + r_base) < j0) dead_r = r_base;
                 }
                 if (r_base == dead_r) {  // the whole round lies behind a known miss
-                    if (active && hl) hl[g] = CW_MISS;
+                    if (active && hl) __stcs(hl + g, CW_MISS);
                     continue;
                 }
             }
@@ -344,7 +344,7 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
                     if (loc & CW_HOST_BIT) atomicAdd(&host_hits[r], 1u);
                 }
             }
-            if (active && hl) hl[g] = loc;
+            if (active && hl) __stcs(hl + g, loc);
         }
     }
 }

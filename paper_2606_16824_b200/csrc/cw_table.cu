@@ -241,7 +241,8 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
             {
                 u64 kk[KPL];
 #pragma unroll
-                for (int q = 0; q < KPL; ++q) kk[q] = lane + 32 * q < n_task ? hs[c0 + lane + 32 * q] : 0;  // in flight together
+                for (int q = 0; q < KPL; ++q)  // in flight together; streaming (evict-first): the table stays in L2
+                    kk[q] = lane + 32 * q < n_task ? __ldcs(hs + c0 + lane + 32 * q) : 0;
 #pragma unroll
                 for (int q = 0; q < KPL; ++q) wkey[lane + 32 * q] = cw_remap_key(kk[q]);  // read back by this lane only
             }

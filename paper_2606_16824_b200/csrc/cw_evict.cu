@@ -437,22 +437,23 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
         const u32 s0 = tau_smem ? tid : blockIdx.x * CWE_THREADS + tid;
         const u32 sstep = tau_smem ? CWE_THREADS : G * CWE_THREADS;
         for (u32 s = s0; s < a.S; s += sstep) {
+            // the predictor inputs are requested together with the session state (one memory latency, not two)
             const u32 stt = a.session_state[s];
-            u32 tau;
-            if (stt == CW_SESSION_QUEUED || stt == CW_SESSION_RUNNING) {
-                tau = 0;
-            } else if (stt >= CW_SESSION_IDLE) {
-                tau = CW_TAU_MAX;
-            } else if (a.tau_override) {
-                tau = min(a.tau_override[s], CW_TAU_MAX - 1);
+            i32 raw = a.bias;
+            u32 ov = 0;
+            if (a.tau_override) {
+                ov = a.tau_override[s];
             } else {
-                i32 raw = a.bias;
                 const uint8_t* x = a.features + (u64)s * a.F;
 #pragma unroll
-                for (u32 f = 0; f < 16; ++f)  // F <= 16: predicated, independent loads (one latency, not F)
+                for (u32 f = 0; f < 16; ++f)  // F <= 16: predicated, independent loads
                     if (f < a.F) raw += (i32)a.weights[f] * (i32)x[f];
-                tau = (u32)min(max(raw, 0), (i32)(CW_TAU_MAX - 1));
             }
+            u32 tau;
+            if (stt == CW_SESSION_QUEUED || stt == CW_SESSION_RUNNING) tau = 0;
+            else if (stt >= CW_SESSION_IDLE) tau = CW_TAU_MAX;
+            else if (a.tau_override) tau = min(ov, CW_TAU_MAX - 1);
+            else tau = (u32)min(max(raw, 0), (i32)(CW_TAU_MAX - 1));
             if (tau_smem) s_tau[s] = tau;
             else a.tau_q[s] = tau;
             const u32 v = CW_TAU_MAX - tau;

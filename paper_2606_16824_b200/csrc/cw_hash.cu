@@ -152,7 +152,7 @@ __global__ void __launch_bounds__(1024) hash_plan_kernel(const HashArgs a) {
 }
 
 // ------------------------------------------------------------------------------------------------ main pass
-__global__ void __launch_bounds__(CWH_UNIT + 32, 4) hash_kernel(const HashArgs a) {
+__global__ void __launch_bounds__(CWH_UNIT + 32, CWH_MIN_CTAS) hash_kernel(const HashArgs a) {
     extern __shared__ __align__(128) uint8_t smem_raw[];
     HashSmem& sm = *reinterpret_cast<HashSmem*>(smem_raw);
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;

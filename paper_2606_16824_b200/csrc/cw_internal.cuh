@@ -61,7 +61,12 @@ __host__ __device__ __forceinline__ u64 cw_remap_key(u64 k) {
 #define CWH_WARPS 8                   // consumer warps per CTA
 #define CWH_UNIT (32 * CWH_WARPS)     // blocks per unit (one unit = one CTA iteration)
 #define CWH_UNIT_LOG2 8
+#ifndef CWH_STAGES
 #define CWH_STAGES 3                  // smem ring depth
+#endif
+#ifndef CWH_MIN_CTAS
+#define CWH_MIN_CTAS 4
+#endif
 #define CWH_STAGE_BYTES (CWH_UNIT * 64 + 16)
 
 struct cw_hash_rec {  // what the CTA of one range publishes for the CTA of the next range

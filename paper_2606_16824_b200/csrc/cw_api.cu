@@ -42,7 +42,6 @@ void free_all(cw_ctx* c) {
     cudaFree(c->m_max_hit);
     cudaFree(c->m_host_hits);
     cudaFree(c->sched_a);
-    cudaFree(c->sched_ticket);
     cudaFree(c->tau_q);
     cudaFree(c->out_score);
     cudaFree(c->out_id);
@@ -50,6 +49,7 @@ void free_all(cw_ctx* c) {
     cudaFree(c->ev);
     cudaFree(c->ev_bhist);
     cudaFree(c->ev_boff);
+    cudaFree(c->ev_brec);
     cudaFree(c->ev_bcur);
     cudaFree(c->ev_blist);
     cudaFree(c->staging);
@@ -125,7 +125,6 @@ int32_t cw_create(const cw_config* cfg, cw_ctx** out) {
     CW_CUDA(c, dalloc_zero(&c->m_host_hits, cfg->max_requests, s));
     // stage 2b
     CW_CUDA(c, dalloc_zero(&c->sched_a, cfg->max_requests, s));
-    CW_CUDA(c, dalloc_zero(&c->sched_ticket, 1, s));
     // stage 3
     c->ev_cap = cfg->num_blocks > cfg->host_slots ? cfg->num_blocks : cfg->host_slots;
     CW_CUDA(c, dalloc_zero(&c->tau_q, cfg->max_sessions ? cfg->max_sessions : 1, s));
@@ -139,6 +138,7 @@ int32_t cw_create(const cw_config* cfg, cw_ctx** out) {
     CW_CUDA(c, dalloc_zero(&c->ev, 1, s));
     CW_CUDA(c, dalloc_zero(&c->ev_bhist, 65536 + 128, s));
     CW_CUDA(c, dalloc_zero(&c->ev_boff, 65537, s));
+    CW_CUDA(c, dalloc_zero(&c->ev_brec, 65536, s));
     CW_CUDA(c, dalloc_zero(&c->ev_bcur, 65536, s));
     CW_CUDA(c, dalloc_zero(&c->ev_blist, 196608, s));
     // stage 4

@@ -58,6 +58,7 @@ struct EvictArgs {
     u64* out_score;
     u32* out_id;
     u32* bhist;      // phase D: victims per bucket, exclusive scan, scatter cursors, bucket work lists
+    u64* brec;       // phase D: one record per non-empty bucket: first position << 32 | min(size, 0xFFFF) << 16 | bucket
     u32* boff;
     u32* bcur;
     u32* blist;
@@ -300,7 +301,8 @@ __device__ __forceinline__ void tile_append(const bool (&f0)[CWE_ITEMS], const b
 }
 
 // block-wide OR of N (u64,u32) pairs of masks into accumulators in global (or shared) memory: hardware warp
-// reductions (redux.sync), one shared-memory atomic per warp and word, one atomic per CTA and word at the target
+// reductions (redux.sync), per-warp partials in shared memory folded by one warp per word, one atomic per CTA and
+// word at the target
 template <int N>
 __device__ __forceinline__ void block_or_n(const u64 (&hi)[N], const u32 (&lo)[N], u64* const (&g_hi)[N],
                                            u32* const (&g_lo)[N], u64* s_hi, u32* s_lo) {
@@ -606,20 +608,35 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
                         const u32 thr = s_thr[0], before = s_thr[1], inside = s_thr[2];
                         const u32 need_here = remaining - before;
                         const bool take_all = need_here == inside;
-                        for (u32 i = tid; i < n; i += CWE_THREADS) {
-                            const u64 ms = c_s[i];
-                            const u32 mi = c_i[i];
-                            const u32 dg = plan_digit(lp, ms, mi);
-                            if (dg < thr || (take_all && dg == thr)) {
-                                const u32 pos = base + emitted + atomicAdd(&s_cnt[0], 1u);
+                        for (u32 i0 = 0; i0 < n; i0 += CWE_THREADS) {  // warp-uniform trip count
+                            const u32 i = i0 + tid;
+                            const bool ok = i < n;
+                            const u64 ms = ok ? c_s[i] : 0ull;
+                            const u32 mi = ok ? c_i[i] : 0u;
+                            const u32 dg = ok ? plan_digit(lp, ms, mi) : 0xFFFFFFFFu;
+                            const bool out = ok && (dg < thr || (take_all && dg == thr));
+                            const bool keep = ok && !out && dg == thr;
+                            // one returning shared-memory atomic per warp and list (per-element returning atomics on
+                            // one counter serialise: this loop was most of the CTA-local finish)
+                            const u32 lane = tid & 31, lt = (1u << lane) - 1;
+                            const u32 bo = __ballot_sync(0xffffffffu, out), bk = __ballot_sync(0xffffffffu, keep);
+                            u32 po = 0, pk = 0;
+                            if (lane == 0) {
+                                if (bo) po = atomicAdd(&s_cnt[0], (u32)__popc(bo));
+                                if (bk) pk = atomicAdd(&s_cnt[1], (u32)__popc(bk));
+                            }
+                            po = __shfl_sync(0xffffffffu, po, 0);
+                            pk = __shfl_sync(0xffffffffu, pk, 0);
+                            if (out) {
+                                const u32 pos = base + emitted + po + __popc(bo & lt);
                                 a.out_score[pos] = ms;
                                 a.out_id[pos] = mi;
                                 v_or_hi |= ms;
                                 v_nand_hi |= ~ms;
                                 v_or_lo |= mi;
                                 v_nand_lo |= ~mi;
-                            } else if (dg == thr) {
-                                const u32 pos = atomicAdd(&s_cnt[1], 1u);
+                            } else if (keep) {
+                                const u32 pos = pk + __popc(bk & lt);
                                 n_s[pos] = ms;
                                 n_i[pos] = mi;
                             }
@@ -854,7 +871,9 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
             u32 lbase = 0;
             if (lane == 0 && ne) lbase = atomicAdd(&st->n_nonempty, (u32)__popc(ne));
             lbase = __shfl_sync(0xffffffffu, lbase, 0);
-            if (mine != 0) a.blist[2 * CWE_BUCKETS + lbase + __popc(ne & ((1u << lane) - 1))] = first + tid;
+            if (mine != 0)  // everything the bucket's sorter needs in one load
+                a.brec[lbase + __popc(ne & ((1u << lane) - 1))] =
+                    ((u64)(s_base[0] + s_scan[warp] + inc - mine) << 32) | ((u64)min(mine, 0xFFFFu) << 16) | (first + tid);
         }
         if (blockIdx.x == 0 && tid == 0) {
             a.boff[CWE_BUCKETS] = want;
@@ -896,8 +915,10 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
         const u32 n_nonempty = __ldcg(&st->n_nonempty);
         {
           for (u32 q = gw; q < n_nonempty; q += nw) {
-            const u32 d = __ldcg(a.blist + 2 * CWE_BUCKETS + q);
-            const u32 b0 = __ldcg(a.boff + d), n = __ldcg(a.boff + d + 1) - b0;
+            const u64 rec = __ldcg(a.brec + q);
+            const u32 d = (u32)rec & 0xFFFFu, b0 = (u32)(rec >> 32);
+            u32 n = (u32)(rec >> 16) & 0xFFFFu;
+            if (n == 0xFFFFu) n = __ldcg(a.boff + d + 1) - b0;  // saturated size field
             if (lane == 0) a.bhist[d] = 0;  // self-cleaning
             if (n == 1) {
                 if (lane == 0) {
@@ -1042,6 +1063,7 @@ int32_t cwi_score_evict(cw_ctx* ctx, u32 tick_now, u32 S, u32 F, const uint8_t* 
     a.out_score = ctx->out_score;
     a.out_id = ctx->out_id;
     a.bhist = ctx->ev_bhist;
+    a.brec = ctx->ev_brec;
     a.boff = ctx->ev_boff;
     a.bcur = ctx->ev_bcur;
     a.blist = ctx->ev_blist;

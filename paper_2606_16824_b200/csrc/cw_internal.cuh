@@ -134,7 +134,6 @@ struct cw_ctx {
     u32* m_host_hits;
     // stage 2b
     u32* sched_a;       // a of every request in dispatch order (max_requests)
-    u32* sched_ticket;  // "last CTA done" counter, self-cleaning
     // stage 3
     u32* tau_q;
     u64* cand_score[2];
@@ -145,6 +144,7 @@ struct cw_ctx {
     cw_evict_state* ev;
     u32* ev_bhist;   // victims per bucket (CWE_BUCKETS) + per slice of 512 buckets (128)
     u32* ev_boff;    // exclusive scan (CWE_BUCKETS + 1)
+    u64* ev_brec;    // one record per non-empty bucket (CWE_BUCKETS)
     u32* ev_bcur;    // scatter cursors (CWE_BUCKETS)
     u32* ev_blist;   // [0, 65536): medium buckets, [65536, 131072): large, [131072, 196608): non-empty
     u32 ev_cap;

@@ -81,15 +81,8 @@ __global__ void __launch_bounds__(CWS_MAX_THREADS)
     bool done = false;
     if (R <= CWS_FAST_KEYS * n_thr) {
         u32* s_c = reinterpret_cast<u32*>(s_k0);
-        __shared__ u32 s_mm[4];
+        __shared__ u32 s_mm[4][CWS_MAX_I];  // per-warp partial min / max (no shared-memory atomics: they serialise)
         __shared__ u32 s_tie[CWS_MAX_I][CWS_TIE_CAP];
-        if (tid == 0) {
-            s_mm[0] = 0xFFFFFFFFu;
-            s_mm[1] = 0;
-            s_mm[2] = 0xFFFFFFFFu;
-            s_mm[3] = 0;
-        }
-        __syncthreads();
         u32 hi[CWS_FAST_KEYS], lo[CWS_FAST_KEYS];
         u32 hmin = 0xFFFFFFFFu, hmax = 0, lmin = 0xFFFFFFFFu, lmax = 0;
         // unconditional loads at clamped indices (policy hoisted): all of a thread's loads are in flight together
@@ -132,15 +125,20 @@ __global__ void __launch_bounds__(CWS_MAX_THREADS)
         lmin = __reduce_min_sync(0xffffffffu, lmin);
         lmax = __reduce_max_sync(0xffffffffu, lmax);
         if (jl == 0) {
-            atomicMin(&s_mm[0], hmin);
-            atomicMax(&s_mm[1], hmax);
-            atomicMin(&s_mm[2], lmin);
-            atomicMax(&s_mm[3], lmax);
+            s_mm[0][il] = hmin;
+            s_mm[1][il] = hmax;
+            s_mm[2][il] = lmin;
+            s_mm[3][il] = lmax;
         }
         __syncthreads();
-        hmin = s_mm[0];
-        lmin = s_mm[2];
-        const u32 hb = 32 - __clz(s_mm[1] - hmin), lb = 32 - __clz(s_mm[3] - lmin);
+        {   // every warp folds the per-warp partials on its own (32 lanes, 4 redux): no second barrier
+            const u32 nw = n_thr >> 5;
+            hmin = __reduce_min_sync(0xffffffffu, jl < nw ? s_mm[0][jl] : 0xFFFFFFFFu);
+            hmax = __reduce_max_sync(0xffffffffu, jl < nw ? s_mm[1][jl] : 0u);
+            lmin = __reduce_min_sync(0xffffffffu, jl < nw ? s_mm[2][jl] : 0xFFFFFFFFu);
+            lmax = __reduce_max_sync(0xffffffffu, jl < nw ? s_mm[3][jl] : 0u);
+        }
+        const u32 hb = 32 - __clz(hmax - hmin), lb = 32 - __clz(lmax - lmin);
         if (hb + lb <= 30) {  // CTA-uniform
             done = true;
             const u32 n_pad = (R + 127) & ~127u;  // one warp-wide LDS.128 covers 128 keys; pad never compares below
@@ -343,9 +341,14 @@ __global__ void __launch_bounds__(CWA_THREADS)
             }
         }
     }
-    if (cnt) {
-        atomicAdd(&s_count, cnt);
-        atomicMax(&s_need, (unsigned long long)last_need);
+    {   // one shared-memory atomic per warp, not per thread
+        const u32 wc = __reduce_add_sync(0xffffffffu, cnt);
+        const u32 nh = __reduce_max_sync(0xffffffffu, (u32)(last_need >> 32));
+        const u32 nl = __reduce_max_sync(0xffffffffu, (u32)(last_need >> 32) == nh ? (u32)last_need : 0u);
+        if (lane == 0 && wc) {
+            atomicAdd(&s_count, wc);
+            atomicMax(&s_need, ((unsigned long long)nh << 32) | nl);
+        }
     }
     __syncthreads();
     if (tid == 0) {

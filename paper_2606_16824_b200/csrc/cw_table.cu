@@ -13,12 +13,16 @@
 // (All same-key threads follow one probe sequence whose slots only go from reusable to occupied during the
 // batch, so they converge on the same slot.)
 //
-// Match: one lane per hash, flat over hashes[]; a warp task is 128 consecutive hashes (one 32-ary search over
-// hash_off for its first request, then a sequential walk; rounds that lie behind a miss already seen for their
-// request are answered without a probe).  Per request: first_miss = atomicMin over missing lanes, max_hit =
-// atomicMax over hits that are not already behind a miss of their own round; a small per-request kernel then
-// writes k_total / n_gpu and blanks hits that lie behind the first miss (rare), and re-arms the scratch for the
-// next call.
+// Match: flat over hashes[]; a warp task is 128 consecutive hashes (one 32-ary search over hash_off for its first
+// request).  A task inside one request is probed LANE-INDEPENDENTLY: lane l owns hashes l + 32k, keys and results are
+// staged per warp in shared memory, every iteration of a warp-synchronous loop issues one slot load per live lane and
+// each lane walks its own keys front to back; the first missing position is min-reduced over the warp and lanes stop
+// at it.  Tasks that cross a request boundary walk round by round (32 hashes, one lane per hash); rounds that lie behind
+// a miss already seen for their request are answered without a probe.  Per request: first_miss = atomicMin, max_hit =
+// atomicMax over hits that are not already behind a miss of their own task / round; a small per-request kernel then
+// writes k_total / n_gpu and blanks hits that lie behind the first miss (rare), and re-arms the scratch for the next
+// call.  hit_loc is written with streaming stores and the hashes are read with streaming loads: neither is re-read
+// by this pass, and the table should own the L2.
 #include <stdio.h>
 
 #include "cw_internal.cuh"

@@ -36,8 +36,8 @@ PCIE_GEN5_X16_GBS = 63.0  # 32 GT/s x 16 lanes x 128/130 / 8 per direction (SURV
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r1_full_step_kernels.md), full-size configs[2] step.
-NCU_TRAFFIC_BYTES = {"hash": 434_312_192, "match": 102_913_536, "score_evict": 17_157_632, "gather": 1_659_608_319,
-                     "scatter": 1_659_384_832, "schedule": 126_207}
+NCU_TRAFFIC_BYTES = {"hash": 434_061_567, "match": 94_640_384, "score_evict": 17_158_400, "gather": 1_660_499_200,
+                     "scatter": 1_658_865_408, "schedule": 126_976}
 
 
 def measured_peaks():

@@ -17,7 +17,8 @@
 //          CTA that is waited for has always started: the single wait per CTA cannot deadlock and happens
 //          when both CTAs are finishing anyway.
 //
-// Two launches per call:
+// Two launches per call (one for calls of at most CWH_SMALL_R requests — the steady-state step — where every CTA of
+// hash_kernel rebuilds the plan in shared memory and the last CTA to finish re-arms the ticket and the epoch):
 //   hash_plan_kernel   units per request -> exclusive scan unit_off[R+1]; validates the offsets
 //   hash_kernel        the streaming pass: one producer warp issues ONE TMA bulk copy (cp.async.bulk, L2
 //                      evict-first) of each unit's 16 KiB of token ids into a 3-stage shared-memory ring
@@ -46,11 +47,12 @@ struct HashArgs {
     const u64* hash_off;
     u64* hashes;
     u64* unit_off;      // [R+1] exclusive scan of units per request
-    u64* plan;          // [0] total units, [1] call epoch, [2] range ticket
+    u64* plan;          // [0] total units, [1] call epoch, [2] range ticket, [3] CTAs done (small calls)
     cw_hash_rec* rec;   // per CTA of hash_kernel
     u32* status;
     u64 max_hashed;
     u32 R;
+    u32 small;          // R <= CWH_SMALL_R: no plan kernel, every CTA rebuilds the plan in shared memory
 };
 
 enum { MODE_CONTINUE = 0, MODE_SEED = 1, MODE_ZERO = 2 };
@@ -74,6 +76,8 @@ struct __align__(128) HashSmem {
     u64 wagg[2][CWH_WARPS];
     u64 pw[CWH_WARPS + 1];  // (A^32)^k
     u64 carry_in;
+    u32 uoff[CWH_SMALL_R + 1];  // small calls: exclusive scan of units per request
+    u32 wsum[CWH_WARPS + 1];
     u32 range;
     u32 rec_flags;
     u32 rec_bseg_len;
@@ -158,13 +162,73 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, CWH_MIN_CTAS) hash_kernel(const
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     if (tid == 0) sm.range = atomicAdd(reinterpret_cast<unsigned int*>(a.plan + 2), 1u);
+    const bool small = a.small != 0;
+    u64 U;
+    u32 epoch;
+    if (small) {
+        // ---- small call (R <= CWH_SMALL_R, the steady-state step): no plan kernel.  Every CTA computes the units of
+        // every request (two per thread, one round of loads), scans them and keeps the offsets in shared memory; the
+        // last CTA to finish re-arms the ticket and advances the epoch.
+        const u32 R = a.R;
+        const bool too_big = a.hash_off[R] < a.hash_off[0] || a.hash_off[R] - a.hash_off[0] > a.max_hashed;
+        u32 t2[2];
+        bool bad = too_big;
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            const u32 r = tid * 2 + k;
+            u64 T = r < R ? plan_units(a, r, too_big) : 0;
+            if (T == ~0ull) {
+                bad = true;
+                T = 0;
+            }
+            t2[k] = (u32)T;
+        }
+        if (bad && blockIdx.x == 0) atomicOr(a.status, CWS_INVAL);
+        const u32 local = t2[0] + t2[1];
+        u32 inc = local;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const u32 y = __shfl_up_sync(0xffffffffu, inc, d);
+            if (lane >= (u32)d) inc += y;
+        }
+        if (lane == 31) sm.wsum[warp] = inc;
+        __syncthreads();
+        u32 before = 0, total = 0;
+#pragma unroll
+        for (u32 w = 0; w <= CWH_WARPS; ++w) {
+            const u32 v = sm.wsum[w];
+            if (w < warp) before += v;
+            total += v;
+        }
+        const u32 excl = before + inc - local;
+        if (tid * 2 < R) sm.uoff[tid * 2] = excl;
+        if (tid * 2 + 1 < R) sm.uoff[tid * 2 + 1] = excl + t2[0];
+        if (tid == 0) sm.uoff[R] = total;
+        U = total;
+        epoch = (u32)a.plan[1] + 1;
+    } else {
+        U = a.plan[0];
+        epoch = (u32)a.plan[1];
+    }
     __syncthreads();
+    auto uo = [&](u32 i) -> u64 { return small ? (u64)sm.uoff[i] : a.unit_off[i]; };
+    auto call_done = [&]() {  // self-cleaning: the last CTA re-arms the ticket (a small call may follow without a plan
+        if (tid == 0) {       // kernel) and, in a small call, advances the epoch
+            const u32 old = atomicAdd(reinterpret_cast<unsigned int*>(a.plan + 3), 1u);
+            if (old == gridDim.x - 1) {
+                a.plan[3] = 0;
+                a.plan[2] = 0;
+                if (small) a.plan[1] = a.plan[1] + 1;
+            }
+        }
+    };
     const u32 range = sm.range;  // ranges in ticket order: every lower range belongs to a CTA that has started
-    const u64 U = a.plan[0];
-    const u32 epoch = (u32)a.plan[1];
     const u64 per = (U + gridDim.x - 1) / gridDim.x;
     const u64 u_begin = min(U, per * range), u_end = min(U, u_begin + per);
-    if (u_begin >= u_end) return;  // empty range (uniform over the CTA): nobody waits for it
+    if (u_begin >= u_end) {  // empty range (uniform over the CTA): nobody waits for it
+        call_done();
+        return;
+    }
 
     if (tid <= CWH_WARPS) sm.pw[tid] = pow_u64(cw_pow(CW_A, 32), tid);
     if (tid == 0) {
@@ -184,7 +248,7 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, CWH_MIN_CTAS) hash_kernel(const
         while (hi - lo > 1) {
             u32 step = (hi - lo + 31) >> 5;
             u32 p = lo + lane * step;
-            bool ok = p < hi && a.unit_off[p] <= u_begin;
+            bool ok = p < hi && uo(p) <= u_begin;
             u32 cnt = __popc(__ballot_sync(0xffffffffu, ok));
             u32 nlo = lo + (cnt - 1) * step;
             hi = min(hi, nlo + step);
@@ -194,7 +258,7 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, CWH_MIN_CTAS) hash_kernel(const
             const u64 policy = policy_evict_first();
             u32 r = lo;
             u64 u = u_begin;
-            u64 uo0 = a.unit_off[r], uo1 = a.unit_off[r + 1];
+            u64 uo0 = uo(r), uo1 = uo(r + 1);
             u64 t = u - uo0;
             const bool starts_mid = t > 0;  // the first request began in an earlier CTA's range
             bool in_bseg = starts_mid;
@@ -239,7 +303,7 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, CWH_MIN_CTAS) hash_kernel(const
                     do {
                         ++r;
                         uo0 = uo1;
-                        uo1 = a.unit_off[r + 1];
+                        uo1 = uo(r + 1);
                     } while (uo1 == uo0);  // requests without work
                     t = 0;
                     fresh = true;
@@ -374,6 +438,7 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, CWH_MIN_CTAS) hash_kernel(const
                 const i32 k = k_hi - (i32)lane;
                 const cw_hash_rec* prev = a.rec + (k >= 0 ? k : 0);
                 u32 nuse;
+                bool fin_found;
                 for (;;) {  // poll until the records from k_hi down to the first final one are all published
                     const bool ready = k < 0 || ld_acquire_u32(&prev->ready) == epoch;
                     const bool fin = k < 0 || (ready && !(*reinterpret_cast<const volatile u32*>(&prev->len_kind) & 0x80000000u));
@@ -382,7 +447,8 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, CWH_MIN_CTAS) hash_kernel(const
                     const u32 first_fin = fmask ? (u32)__ffs(fmask) - 1 : 32u;
                     const u32 need = first_fin >= 32 ? 0xffffffffu : ((2u << first_fin) - 1);  // lanes 0..first_fin
                     if ((rmask & need) == need) {
-                        nuse = first_fin >= 32 ? 32u : first_fin + 1;
+                        fin_found = first_fin < 32;
+                        nuse = fin_found ? first_fin + 1 : 32u;
                         break;
                     }
                 }
@@ -404,7 +470,7 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, CWH_MIN_CTAS) hash_kernel(const
 #pragma unroll
                 for (int d = 16; d; d >>= 1) term += shfl64_xor(term, d);
                 carry_in += term;
-                if (nuse < 32 || k_hi < 32) break;  // reached a final record (range 0 is always final)
+                if (fin_found) break;  // reached a final record (range 0 is always final; k < 0 counts as final)
                 mult *= shfl64(incl, 31);
                 k_hi -= 32;
             }
@@ -422,6 +488,7 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, CWH_MIN_CTAS) hash_kernel(const
             m *= stride;
         }
     }
+    call_done();
 }
 
 }  // namespace
@@ -451,8 +518,11 @@ int32_t cwi_hash_blocks(cw_ctx* ctx, const i32* d_tokens, const u64* d_tok_off, 
     a.status = ctx->d_status;
     a.max_hashed = ctx->cfg.max_hashed_blocks;
     a.R = R;
-    hash_plan_kernel<<<1, 1024, 0, ctx->s_main>>>(a);
-    CW_LAUNCH_CHECK(ctx);
+    a.small = R <= CWH_SMALL_R ? 1u : 0u;
+    if (!a.small) {
+        hash_plan_kernel<<<1, 1024, 0, ctx->s_main>>>(a);
+        CW_LAUNCH_CHECK(ctx);
+    }
     // never more CTAs than units could exist; small calls stay small
     u64 max_units = (ctx->cfg.max_hashed_blocks >> CWH_UNIT_LOG2) + R;
     int grid = (int)((u64)ctx->hash_grid < max_units ? (u64)ctx->hash_grid : max_units);

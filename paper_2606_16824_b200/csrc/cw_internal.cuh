@@ -61,6 +61,7 @@ __host__ __device__ __forceinline__ u64 cw_remap_key(u64 k) {
 #define CWH_WARPS 8                   // consumer warps per CTA
 #define CWH_UNIT (32 * CWH_WARPS)     // blocks per unit (one unit = one CTA iteration)
 #define CWH_UNIT_LOG2 8
+#define CWH_SMALL_R 512                // calls with at most this many requests skip the plan kernel
 #ifndef CWH_STAGES
 #define CWH_STAGES 3                  // smem ring depth
 #endif

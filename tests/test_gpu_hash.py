@@ -120,3 +120,20 @@ def test_host_side_argument_checks(ctx):
         assert e.value.code == cw.CW_E_INVAL
     ctx.hash_blocks(tok, off, ho, 0, out)  # R = 0 is a no-op
     assert ctx.sync(check=False) == 0
+
+
+def test_small_and_large_calls_interleaved_on_one_context():
+    """Calls of at most 512 requests rebuild the plan inside the hash kernel (no plan kernel) and re-arm the range
+    ticket and the epoch themselves; larger calls go through the plan kernel.  Any order of the two on one context,
+    including long requests that span many ranges (look-back over dependent ranges), must stay bit-exact."""
+    from gpu_util import small_ctx
+    ctx = small_ctx(max_requests=4096, max_hashed_blocks=1 << 21)
+    g = gen.rng(41, 0)
+    for rnd, R in enumerate([3, 700, 1, 512, 513, 2, 2, 900, 511, 40]):
+        lens = g.integers(0, 600, size=R)
+        lens[g.integers(0, R)] = int(g.integers(100_000, 400_000))     # one request over hundreds of units
+        tok_off = np.concatenate([[0], np.cumsum(lens)]).astype(np.uint64)
+        tokens = g.integers(0, gen.VOCAB, size=int(tok_off[-1]), dtype=np.int32)
+        salt = g.integers(0, 2**63, size=R, dtype=np.uint64) if rnd % 2 else None
+        _check(ctx, tokens, tok_off, **({"salt": salt} if salt is not None else {}))
+    ctx.close()

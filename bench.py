@@ -36,8 +36,8 @@ PCIE_GEN5_X16_GBS = 63.0  # 32 GT/s x 16 lanes x 128/130 / 8 per direction (SURV
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r1_full_step_kernels.md), full-size configs[2] step.
-NCU_TRAFFIC_BYTES = {"hash": 434_061_567, "match": 94_640_384, "score_evict": 17_158_400, "gather": 1_660_499_200,
-                     "scatter": 1_658_865_408, "schedule": 126_976}
+NCU_TRAFFIC_BYTES = {"hash": 434_067_199, "match": 94_296_064, "score_evict": 17_158_912, "gather": 1_660_988_672,
+                     "scatter": 1_659_497_727, "schedule": 126_976}
 
 
 def measured_peaks():

@@ -912,10 +912,11 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
         u32* wi = s_id + warp * 128;
         // warp w of CTA c takes buckets c + G*w, ...: the few thousand busy warps are spread over all SMs
         const u32 gw = warp * G + blockIdx.x, nw = (G * CWE_THREADS) >> 5;
+        const u64 rec_first = __ldcg(a.brec + gw);  // speculative (gw < 65536): in flight together with the count
         const u32 n_nonempty = __ldcg(&st->n_nonempty);
         {
           for (u32 q = gw; q < n_nonempty; q += nw) {
-            const u64 rec = __ldcg(a.brec + q);
+            const u64 rec = q == gw ? rec_first : __ldcg(a.brec + q);
             const u32 d = (u32)rec & 0xFFFFu, b0 = (u32)(rec >> 32);
             u32 n = (u32)(rec >> 16) & 0xFFFFu;
             if (n == 0xFFFFu) n = __ldcg(a.boff + d + 1) - b0;  // saturated size field

@@ -84,9 +84,13 @@ int32_t cw_sync(cw_ctx* ctx);
 int32_t cw_join_copy(cw_ctx* ctx);
 /* Text of the last CW_E_CUDA failure ("" if none).  Valid until the next call on this ctx. */
 const char* cw_last_error(cw_ctx* ctx);
-/* Diagnostics: waits for stream_main, then copies the 32 device timestamps (ns, %globaltimer) that CTA 0 of the
- * last cw_score_evict took after each of its grid-wide phases; h_out32[31] = how many are valid. */
+#ifdef CW_DEBUG
+/* Debug builds only (libcachewise_debug.so, -DCW_DEBUG; not part of the product ABI).  Waits for stream_main, then
+ * copies the 32 device timestamps (ns, %globaltimer) that CTA 0 of the last cw_score_evict took after each of its
+ * grid-wide phases; h_out32[31] = how many are valid.  Debug builds also reject duplicate block ids in
+ * cw_swap_out / cw_gather_pages (CW_E_INVAL at cw_sync; SURVEY.md 8c stage 4). */
 int32_t cw_debug_evict_times(cw_ctx* ctx, uint64_t* h_out32);
+#endif
 /* Number of kernels this ctx has launched so far (bench.py's gpu_launches). */
 uint64_t cw_launch_count(const cw_ctx* ctx);
 
@@ -149,6 +153,26 @@ int32_t cw_score_evict(cw_ctx* ctx, uint32_t tick_now, uint32_t S, uint32_t F, c
                        const uint32_t* d_tau_override, const uint32_t* d_deficit, uint32_t tier,
                        uint32_t* d_victims, uint64_t* d_victim_scores, uint32_t* d_num_victims, uint32_t cap);
 
+/* Stage 3, speculative form.  The victims come out SORTED by (score, id), so the victims for any
+ * deficit are a PREFIX of the victims for the step's eviction budget `cap`; the selection therefore does not have to
+ * wait for cw_schedule's deficit.  cw_score_evict_begin forks: the same kernel as cw_score_evict, with deficit = cap,
+ * is launched on a side stream owned by the ctx, ordered after everything queued on stream_main so far; whatever the
+ * caller queues on stream_main next (cw_hash_blocks -> cw_match_prefix -> cw_schedule) runs BESIDE it.
+ * cw_score_evict_end joins: stream_main waits for the side stream, then
+ *     *d_num_victims = min(*d_deficit, cap, #evictable)      (CW_E_CAPACITY latched iff #evictable < min(*d_deficit, cap))
+ * i.e. d_victims[0..*d_num_victims), d_victim_scores and the status are exactly those of cw_score_evict; entries of
+ * d_victims behind *d_num_victims hold the rest of the budget's victims.  Block metadata, the predictor inputs and
+ * the output arrays must not be touched between begin and end.  One begin may be outstanding per ctx (a second one,
+ * or an end without a begin, returns CW_E_STATE).  Both calls can be captured into one CUDA graph on stream_main (the
+ * side stream joins the capture as a parallel branch).
+ *   n_ctas: how many CTAs (= SMs) the speculative kernel may occupy; 0 = library default (a quarter of the SMs, so
+ *   that the kernels on stream_main keep the rest of the machine). */
+int32_t cw_score_evict_begin(cw_ctx* ctx, uint32_t tick_now, uint32_t S, uint32_t F, const uint8_t* d_features,
+                             const int16_t* d_weights, int32_t bias, const uint8_t* d_session_state,
+                             const uint32_t* d_tau_override, uint32_t tier, uint32_t* d_victims,
+                             uint64_t* d_victim_scores, uint32_t cap, uint32_t n_ctas);
+int32_t cw_score_evict_end(cw_ctx* ctx, const uint32_t* d_deficit, uint32_t* d_num_victims);
+
 /* The paper's own predictor (PAPER.md 5.2 L219-225 "expected remaining time for the tool call to complete",
  * L227 per-cluster distributions of historical tool durations).  DESIGN.md reading R7.
  *   d_cluster    uint32[S]: cluster of the tool call each session is waiting on (its metadata class)
@@ -186,7 +210,9 @@ int32_t cw_scatter_pages(cw_ctx* ctx, const uint32_t* d_ids, const uint32_t* d_n
 /* Support calls (used by the host-driven replay).
  * cw_table_insert: keys 0 and 2^64-1 are remapped to 1 and 2^64-2.  A key already present keeps its loc;
  * among duplicates inside the batch the LOWEST input index wins.  d_winner_loc[i] (may be NULL) = the loc
- * that survives for input i, CW_MISS if the table is full (CW_E_CAPACITY at cw_sync).
+ * that survives for input i, CW_MISS if the table is full (CW_E_CAPACITY at cw_sync).  When the table fills up
+ * the keys that still find a slot are the first ones by input index (a batch that could fill the table is
+ * inserted sequentially; deciding that costs one host sync, so such a call cannot be captured: CW_E_STATE).
  * cw_table_erase: absent keys are a no-op.  cw_table_retag: sets loc of present keys (keys must be distinct).
  * cw_table_lookup: d_loc[i] = loc or CW_MISS. */
 int32_t cw_table_insert(cw_ctx* ctx, const uint64_t* d_keys, const uint32_t* d_loc, uint32_t n,
@@ -194,6 +220,15 @@ int32_t cw_table_insert(cw_ctx* ctx, const uint64_t* d_keys, const uint32_t* d_l
 int32_t cw_table_erase(cw_ctx* ctx, const uint64_t* d_keys, uint32_t n);
 int32_t cw_table_retag(cw_ctx* ctx, const uint64_t* d_keys, const uint32_t* d_new_loc, uint32_t n);
 int32_t cw_table_lookup(cw_ctx* ctx, const uint64_t* d_keys, uint32_t n, uint32_t* d_loc);
+/* Table maintenance (R2b).  Erases leave tombstones; cw_table_erase compacts the table on its own once
+ * the erases since the last compaction could have turned a quarter of the slots into tombstones (not while
+ * stream_main is being captured).  cw_table_compact forces it: live entries are re-inserted into a second buffer
+ * and copied back (the table keeps its address).
+ * cw_table_stats: waits for stream_main; h_out8 = { live keys, tombstones, slots, longest probe, median probe, p99
+ * probe, compactions so far, sum of probe lengths }, a probe length being the slots examined to find a resident key
+ * (lengths above 1024 are counted as 1024 in the median / p99 / sum). */
+int32_t cw_table_compact(cw_ctx* ctx);
+int32_t cw_table_stats(cw_ctx* ctx, uint64_t* h_out8);
 /* cw_blocks_update: scatter per-block metadata of `tier` (0 = HBM blocks, 1 = host slots) at d_ids[0..n);
  * any of the four value arrays may be NULL (= leave unchanged).  PAPER.md 5.3 L250 per-block metadata. */
 int32_t cw_blocks_update(cw_ctx* ctx, uint32_t tier, const uint32_t* d_ids, uint32_t n, const uint32_t* d_session,

@@ -11,7 +11,9 @@ import ctypes as C
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libcachewise.so")
+# CACHEWISE_DEBUG=1 selects the -DCW_DEBUG build (phase timestamps, duplicate-victim check; `build.build(debug=True)`)
+DEBUG = os.environ.get("CACHEWISE_DEBUG", "0") not in ("", "0")
+LIB_PATH = os.path.join(_HERE, "libcachewise_debug.so" if DEBUG else "libcachewise.so")
 
 CW_OK, CW_E_INVAL, CW_E_CAPACITY, CW_E_CUDA, CW_E_STATE = 0, -1, -2, -3, -4
 CW_MISS = 0xFFFFFFFF
@@ -21,10 +23,12 @@ CW_REF_VALID = 0x80000000
 CW_REF_PINNED = 0x40000000
 POLICY_MIN_ADDITIONAL, POLICY_OVERLAP_FIRST, POLICY_FCFS = 0, 1, 2
 
-EXPORTS = ["cw_create", "cw_destroy", "cw_sync", "cw_join_copy", "cw_debug_evict_times", "cw_last_error", "cw_launch_count", "cw_hash_blocks",
-           "cw_match_prefix", "cw_schedule", "cw_score_evict", "cw_predict_tau", "cw_swap_out", "cw_swap_in", "cw_gather_pages",
-           "cw_scatter_pages", "cw_table_insert", "cw_table_erase", "cw_table_retag", "cw_table_lookup",
+EXPORTS = ["cw_create", "cw_destroy", "cw_sync", "cw_join_copy", "cw_last_error", "cw_launch_count", "cw_hash_blocks",
+           "cw_match_prefix", "cw_schedule", "cw_score_evict", "cw_score_evict_begin", "cw_score_evict_end",
+           "cw_predict_tau", "cw_swap_out", "cw_swap_in", "cw_gather_pages", "cw_scatter_pages", "cw_table_insert",
+           "cw_table_erase", "cw_table_retag", "cw_table_lookup", "cw_table_compact", "cw_table_stats",
            "cw_blocks_update"]
+DEBUG_EXPORTS = ["cw_debug_evict_times"]  # libcachewise_debug.so only
 
 
 class CwConfig(C.Structure):
@@ -58,7 +62,9 @@ def lib():
         L.cw_destroy.argtypes = [P]
         L.cw_sync.argtypes = [P]
         L.cw_join_copy.argtypes = [P]
-        L.cw_debug_evict_times.argtypes = [P, P]
+        if DEBUG:
+            L.cw_debug_evict_times.argtypes = [P, P]
+            L.cw_debug_evict_times.restype = I32
         L.cw_last_error.argtypes = [P]
         L.cw_last_error.restype = C.c_char_p
         L.cw_launch_count.argtypes = [P]
@@ -67,6 +73,10 @@ def lib():
         L.cw_match_prefix.argtypes = [P, P, P, U32, P, P, P]
         L.cw_schedule.argtypes = [P, U32, P, P, P, P, U32, U32, U32, U32, P, P, P]
         L.cw_score_evict.argtypes = [P, U32, U32, U32, P, P, I32, P, P, P, U32, P, P, P, U32]
+        L.cw_score_evict_begin.argtypes = [P, U32, U32, U32, P, P, I32, P, P, U32, P, P, U32, U32]
+        L.cw_score_evict_end.argtypes = [P, P, P]
+        L.cw_table_compact.argtypes = [P]
+        L.cw_table_stats.argtypes = [P, P]
         L.cw_predict_tau.argtypes = [P, U32, P, P, U32, P, P, P]
         L.cw_swap_out.argtypes = [P, P, P, U32, P, P]
         L.cw_swap_in.argtypes = [P, P, P, P, U32]
@@ -142,7 +152,9 @@ class Context:
         self._ck(lib().cw_join_copy(self._h), "cw_join_copy")
 
     def debug_evict_times(self):
-        """Phase timestamps (ns) of the last score_evict, relative to its first one."""
+        """Phase timestamps (ns) of the last score_evict, relative to its first one (CACHEWISE_DEBUG=1 only)."""
+        if not DEBUG:
+            raise CwError(CW_E_STATE, "cw_debug_evict_times", "needs the debug library (CACHEWISE_DEBUG=1)")
         buf = (C.c_uint64 * 32)()
         self._ck(lib().cw_debug_evict_times(self._h, buf), "cw_debug_evict_times")
         n = min(int(buf[31]), 31)
@@ -172,6 +184,15 @@ class Context:
                                       _ptr(session_state), _ptr(tau_override), _ptr(deficit), tier, _ptr(victims),
                                       _ptr(victim_scores), _ptr(num_victims), cap), "cw_score_evict")
 
+    def score_evict_begin(self, tick_now, S, F, features, weights, bias, session_state, tau_override, tier, victims,
+                          victim_scores, cap, n_ctas=0):
+        self._ck(lib().cw_score_evict_begin(self._h, tick_now, S, F, _ptr(features), _ptr(weights), bias,
+                                            _ptr(session_state), _ptr(tau_override), tier, _ptr(victims),
+                                            _ptr(victim_scores), cap, n_ctas), "cw_score_evict_begin")
+
+    def score_evict_end(self, deficit, num_victims):
+        self._ck(lib().cw_score_evict_end(self._h, _ptr(deficit), _ptr(num_victims)), "cw_score_evict_end")
+
     def predict_tau(self, S, cluster, elapsed_ms, C, sample_off, samples, tau_out):
         self._ck(lib().cw_predict_tau(self._h, S, _ptr(cluster), _ptr(elapsed_ms), C, _ptr(sample_off), _ptr(samples),
                                       _ptr(tau_out)), "cw_predict_tau")
@@ -200,6 +221,16 @@ class Context:
 
     def table_lookup(self, keys, n, loc):
         self._ck(lib().cw_table_lookup(self._h, _ptr(keys), n, _ptr(loc)), "cw_table_lookup")
+
+    def table_compact(self):
+        self._ck(lib().cw_table_compact(self._h), "cw_table_compact")
+
+    def table_stats(self):
+        """dict(live, tombstones, slots, probe_max, probe_p50, probe_p99, compactions, probe_sum); synchronises."""
+        buf = (C.c_uint64 * 8)()
+        self._ck(lib().cw_table_stats(self._h, buf), "cw_table_stats")
+        keys = ("live", "tombstones", "slots", "probe_max", "probe_p50", "probe_p99", "compactions", "probe_sum")
+        return {k: int(buf[i]) for i, k in enumerate(keys)}
 
     def blocks_update(self, tier, ids, n, session=None, depth=None, last_access=None, ref_flags=None):
         self._ck(lib().cw_blocks_update(self._h, tier, _ptr(ids), n, _ptr(session), _ptr(depth), _ptr(last_access),

@@ -21,6 +21,9 @@ cudaError_t dalloc_zero(T** p, size_t n, cudaStream_t s, int fill = 0) {
 
 void free_all(cw_ctx* c) {
     cudaFree(c->table);
+    cudaFree(c->table2);
+    cudaFree(c->tbl_cnt);
+    cudaFree(c->tbl_hist);
     cudaFree(c->ins_slot);
     for (int t = 0; t < 2; ++t) {
         cudaFree(c->meta_session[t]);
@@ -33,6 +36,11 @@ void free_all(cw_ctx* c) {
         if (c->ev_copy[t]) cudaEventDestroy(c->ev_copy[t]);
     }
     if (c->ev_join) cudaEventDestroy(c->ev_join);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_spec) cudaEventDestroy(c->ev_spec);
+    if (c->s_side) cudaStreamDestroy(c->s_side);
+    cudaFree(c->spec_n);
+    cudaFree(c->dup_bits);
     cudaFree(c->d_status);
     if (c->h_status) cudaFreeHost(c->h_status);
     cudaFree(c->hash_unit_off);
@@ -103,6 +111,8 @@ int32_t cw_create(const cw_config* cfg, cw_ctx** out) {
         CW_CUDA(c, cudaMemsetAsync(c->table, 0, c->n_slots * sizeof(cw_slot), s));
         CW_CUDA(c, cudaMemset2DAsync(reinterpret_cast<uint8_t*>(c->table) + 12, sizeof(cw_slot), 0xFF, 4, c->n_slots, s));
     }
+    CW_CUDA(c, dalloc_zero(&c->tbl_cnt, 4, s));
+    CW_CUDA(c, dalloc_zero(&c->tbl_hist, CWT_HIST_BINS, s));
     c->tier_size[0] = cfg->num_blocks;
     c->tier_size[1] = cfg->host_slots;
     for (int t = 0; t < 2; ++t) {
@@ -141,6 +151,19 @@ int32_t cw_create(const cw_config* cfg, cw_ctx** out) {
     CW_CUDA(c, dalloc_zero(&c->ev_brec, 65536, s));
     CW_CUDA(c, dalloc_zero(&c->ev_bcur, 65536, s));
     CW_CUDA(c, dalloc_zero(&c->ev_blist, 196608, s));
+    CW_CUDA(c, dalloc_zero(&c->spec_n, 1, s));
+    {   // function attributes and launch geometry are per DEVICE: set for the device this ctx lives on
+        int32_t st = cwi_evict_init(c);
+        if (st) return st;
+        st = cwi_schedule_init(c);
+        if (st) return st;
+    }
+    CW_CUDA(c, cudaStreamCreateWithFlags(&c->s_side, cudaStreamNonBlocking));
+    CW_CUDA(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+    CW_CUDA(c, cudaEventCreateWithFlags(&c->ev_spec, cudaEventDisableTiming));
+#ifdef CW_DEBUG
+    CW_CUDA(c, dalloc_zero(&c->dup_bits, ((size_t)cfg->num_blocks + 31) / 32, s));
+#endif
     // stage 4
     if (cfg->staging_bytes) {
         if (!cfg->n_chunks || cfg->staging_bytes / 2 < c->page_bytes) {
@@ -164,6 +187,7 @@ int32_t cw_destroy(cw_ctx* ctx) {
     if (!ctx) return CW_E_STATE;
     cudaStreamSynchronize(ctx->s_main);
     if (ctx->s_copy) cudaStreamSynchronize(ctx->s_copy);
+    if (ctx->s_side) cudaStreamSynchronize(ctx->s_side);
     free_all(ctx);
     delete ctx;
     return CW_OK;
@@ -172,6 +196,7 @@ int32_t cw_destroy(cw_ctx* ctx) {
 int32_t cw_sync(cw_ctx* ctx) {
     if (!ctx) return CW_E_STATE;
     CW_CUDA(ctx, cudaStreamSynchronize(ctx->s_copy));
+    CW_CUDA(ctx, cudaStreamSynchronize(ctx->s_side));
     CW_CUDA(ctx, cudaMemcpyAsync(ctx->h_status, ctx->d_status, sizeof(u32), cudaMemcpyDeviceToHost, ctx->s_main));
     CW_CUDA(ctx, cudaMemsetAsync(ctx->d_status, 0, sizeof(u32), ctx->s_main));
     CW_CUDA(ctx, cudaStreamSynchronize(ctx->s_main));
@@ -189,6 +214,7 @@ int32_t cw_join_copy(cw_ctx* ctx) {
     return CW_OK;
 }
 
+#ifdef CW_DEBUG
 int32_t cw_debug_evict_times(cw_ctx* ctx, uint64_t* h_out32) {
     if (!ctx) return CW_E_STATE;
     if (!h_out32) return CW_E_INVAL;
@@ -197,6 +223,7 @@ int32_t cw_debug_evict_times(cw_ctx* ctx, uint64_t* h_out32) {
                             CWE_STAMPS * sizeof(u64), cudaMemcpyDeviceToHost));
     return CW_OK;
 }
+#endif
 
 const char* cw_last_error(cw_ctx* ctx) { return ctx ? ctx->err : "null ctx"; }
 uint64_t cw_launch_count(const cw_ctx* ctx) { return ctx ? ctx->launches : 0; }
@@ -233,19 +260,59 @@ int32_t cw_schedule(cw_ctx* ctx, uint32_t R, const uint32_t* d_need, const uint3
                         d_order, d_num_admit, d_deficit);
 }
 
-int32_t cw_score_evict(cw_ctx* ctx, uint32_t tick_now, uint32_t S, uint32_t F, const uint8_t* d_features,
-                       const int16_t* d_weights, int32_t bias, const uint8_t* d_session_state,
-                       const uint32_t* d_tau_override, const uint32_t* d_deficit, uint32_t tier, uint32_t* d_victims,
-                       uint64_t* d_victim_scores, uint32_t* d_num_victims, uint32_t cap) {
+static int32_t check_evict_args(cw_ctx* ctx, uint32_t S, uint32_t F, const uint8_t* d_features,
+                                const int16_t* d_weights, int32_t bias, const uint8_t* d_session_state,
+                                const uint32_t* d_tau_override, uint32_t tier, const uint32_t* d_victims) {
     if (!ctx) return CW_E_STATE;
-    if (tier > 1 || !d_deficit || !d_victims || !d_num_victims) return CW_E_INVAL;
+    if (tier > 1 || !d_victims) return CW_E_INVAL;
     if (ctx->tier_size[tier] == 0) return CW_E_STATE;
     if (S > ctx->cfg.max_sessions || F > ctx->cfg.max_features || F > 16) return CW_E_INVAL;
     if (bias > (1 << 30) || bias < -(1 << 30)) return CW_E_INVAL;
     if (S && (!d_session_state || (F && !d_tau_override && (!d_features || !d_weights)))) return CW_E_INVAL;
+    return CW_OK;
+}
+
+int32_t cw_score_evict(cw_ctx* ctx, uint32_t tick_now, uint32_t S, uint32_t F, const uint8_t* d_features,
+                       const int16_t* d_weights, int32_t bias, const uint8_t* d_session_state,
+                       const uint32_t* d_tau_override, const uint32_t* d_deficit, uint32_t tier, uint32_t* d_victims,
+                       uint64_t* d_victim_scores, uint32_t* d_num_victims, uint32_t cap) {
+    int32_t st = check_evict_args(ctx, S, F, d_features, d_weights, bias, d_session_state, d_tau_override, tier, d_victims);
+    if (st) return st;
+    if (!d_deficit || !d_num_victims) return CW_E_INVAL;
+    if (ctx->spec_open) return CW_E_STATE;  // the scratch is in use by a speculative selection
     if (cap > ctx->tier_size[tier]) cap = ctx->tier_size[tier];
-    return cwi_score_evict(ctx, tick_now, S, F, d_features, d_weights, bias, d_session_state, d_tau_override,
-                           d_deficit, tier, d_victims, d_victim_scores, d_num_victims, cap);
+    return cwi_score_evict(ctx, ctx->s_main, 0, tick_now, S, F, d_features, d_weights, bias, d_session_state,
+                           d_tau_override, d_deficit, tier, d_victims, d_victim_scores, d_num_victims, cap);
+}
+
+int32_t cw_score_evict_begin(cw_ctx* ctx, uint32_t tick_now, uint32_t S, uint32_t F, const uint8_t* d_features,
+                             const int16_t* d_weights, int32_t bias, const uint8_t* d_session_state,
+                             const uint32_t* d_tau_override, uint32_t tier, uint32_t* d_victims,
+                             uint64_t* d_victim_scores, uint32_t cap, uint32_t n_ctas) {
+    int32_t st = check_evict_args(ctx, S, F, d_features, d_weights, bias, d_session_state, d_tau_override, tier, d_victims);
+    if (st) return st;
+    if (ctx->spec_open) return CW_E_STATE;
+    if (cap > ctx->tier_size[tier]) cap = ctx->tier_size[tier];
+    // fork: the side stream starts after everything queued on stream_main so far
+    CW_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->s_main));
+    CW_CUDA(ctx, cudaStreamWaitEvent(ctx->s_side, ctx->ev_fork, 0));
+    st = cwi_score_evict(ctx, ctx->s_side, n_ctas ? n_ctas : (u32)(ctx->n_sm + 3) / 4, tick_now, S, F, d_features,
+                         d_weights, bias, d_session_state, d_tau_override, nullptr, tier, d_victims, d_victim_scores,
+                         ctx->spec_n, cap);
+    if (st) return st;
+    CW_CUDA(ctx, cudaEventRecord(ctx->ev_spec, ctx->s_side));
+    ctx->spec_open = true;
+    ctx->spec_cap = cap;
+    return CW_OK;
+}
+
+int32_t cw_score_evict_end(cw_ctx* ctx, const uint32_t* d_deficit, uint32_t* d_num_victims) {
+    if (!ctx) return CW_E_STATE;
+    if (!ctx->spec_open) return CW_E_STATE;
+    if (!d_deficit || !d_num_victims) return CW_E_INVAL;
+    CW_CUDA(ctx, cudaStreamWaitEvent(ctx->s_main, ctx->ev_spec, 0));  // join
+    ctx->spec_open = false;
+    return cwi_evict_trim(ctx, d_deficit, ctx->spec_cap, d_num_victims);
 }
 
 int32_t cw_predict_tau(cw_ctx* ctx, uint32_t S, const uint32_t* d_cluster, const uint32_t* d_elapsed_ms, uint32_t C,
@@ -295,9 +362,21 @@ static int32_t pcie_slice(cw_ctx* ctx, uint8_t* half, const uint32_t* h_slots, u
 int32_t cw_swap_out(cw_ctx* ctx, const uint32_t* d_victims, const uint32_t* d_num_victims, uint32_t cap,
                     const uint32_t* h_host_slots, void* h_dst) {
     if (!ctx) return CW_E_STATE;
-    if (!ctx->cfg.n_chunks || !ctx->staging) return CW_E_STATE;
+    if (!ctx->cfg.n_chunks) return CW_E_STATE;
     if (cap == 0) return CW_OK;
     if (!d_victims || !h_dst) return CW_E_INVAL;
+    if (d_num_victims) {
+        // device count: the page count is unknown to the host, so no copy-engine transfer can be sized for it.  The
+        // gather kernel stores straight into the (mapped, pinned) destination: exactly n pages cross PCIe.
+        if (h_host_slots || !cw_aligned16(h_dst)) return CW_E_INVAL;
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, h_dst) != cudaSuccess || at.type != cudaMemoryTypeHost || !at.devicePointer) {
+            cudaGetLastError();
+            return CW_E_INVAL;
+        }
+        return cwi_copy_pages(ctx, ctx->s_main, d_victims, d_num_victims, 0, cap, at.devicePointer, true);
+    }
+    if (!ctx->staging) return CW_E_STATE;
     const u64 page = ctx->page_bytes, half_bytes = (ctx->cfg.staging_bytes / 2) & ~15ull;
     const u32 pps = (u32)(half_bytes / page < 0xFFFFFFFFull ? half_bytes / page : 0xFFFFFFFFull);
     for (u32 first = 0, k = 0; first < cap; first += pps, ++k) {
@@ -305,7 +384,7 @@ int32_t cw_swap_out(cw_ctx* ctx, const uint32_t* d_victims, const uint32_t* d_nu
         const int b = k & 1;
         uint8_t* half = ctx->staging + (u64)b * half_bytes;
         CW_CUDA(ctx, cudaStreamWaitEvent(ctx->s_main, ctx->ev_copy[b], 0));  // PCIe done with this half
-        int32_t st = cwi_copy_pages(ctx, ctx->s_main, d_victims, d_num_victims, first, first + cnt,
+        int32_t st = cwi_copy_pages(ctx, ctx->s_main, d_victims, nullptr, first, first + cnt,
                                     half - (u64)first * page, true);
         if (st) return st;
         CW_CUDA(ctx, cudaEventRecord(ctx->ev_gather[b], ctx->s_main));
@@ -367,6 +446,15 @@ int32_t cw_table_lookup(cw_ctx* ctx, const uint64_t* d_keys, uint32_t n, uint32_
     if (n == 0) return CW_OK;
     if (!d_keys || !d_loc) return CW_E_INVAL;
     return cwi_table_lookup(ctx, d_keys, n, d_loc);
+}
+int32_t cw_table_compact(cw_ctx* ctx) {
+    if (!ctx) return CW_E_STATE;
+    return cwi_table_compact(ctx);
+}
+int32_t cw_table_stats(cw_ctx* ctx, uint64_t* h_out8) {
+    if (!ctx) return CW_E_STATE;
+    if (!h_out8) return CW_E_INVAL;
+    return cwi_table_stats(ctx, h_out8);
 }
 int32_t cw_blocks_update(cw_ctx* ctx, uint32_t tier, const uint32_t* d_ids, uint32_t n, const uint32_t* d_session,
                          const uint32_t* d_depth, const uint32_t* d_last_access, const uint32_t* d_ref_flags) {

@@ -30,9 +30,7 @@ namespace {
 
 #define CWE_THREADS 1024
 #define CWE_WARPS (CWE_THREADS / 32)
-#ifndef CWE_ITEMS
 #define CWE_ITEMS 2  // measured: 2 -> 80 us, 3 -> 82, 4 -> 83, 6 -> 86 (configs[2], whole kernel)
-#endif
 #define CWE_TILE (CWE_THREADS * CWE_ITEMS)
 #define CWE_SMEM_SESS 4096                       // sessions whose tau fits the per-CTA shared-memory table
 #define CWE_SMEM_SORT (CWE_SORT_RUN * 24)        // two (score,id) buffers of the CTA sort (alias the histogram)
@@ -90,11 +88,13 @@ __device__ __forceinline__ void grid_barrier(cw_evict_state* st, u32 nblocks, u3
 
 // phase timestamps of the last call (CTA 0 only; read back by cw_debug_evict_times)
 __device__ __forceinline__ void stamp(cw_evict_state* st, u32& n) {
+#ifdef CW_DEBUG
     if (blockIdx.x == 0 && threadIdx.x == 0 && n < CWE_STAMPS) {
         u64 t;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
         st->stamps[n] = t;
     }
+#endif
     ++n;
 }
 
@@ -521,10 +521,12 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
 
     // ---------------------------------------------------------------- C: radix select
     const u32 n_evictable = __ldcg(&st->n_cand[0]);
-    const u32 asked = min(*a.deficit, a.cap);
+    // a.deficit == NULL: speculative selection of the whole eviction budget (cw_score_evict_begin); the deficit
+    // is applied — and a shortfall reported — by the trim kernel of cw_score_evict_end
+    const u32 asked = a.deficit ? min(*a.deficit, a.cap) : a.cap;
     const u32 want = min(asked, n_evictable);
     if (blockIdx.x == 0 && tid == 0) {
-        if (n_evictable < asked) atomicOr(a.status, CWS_CAPACITY);
+        if (a.deficit && n_evictable < asked) atomicOr(a.status, CWS_CAPACITY);
         *a.num_victims = want;
     }
     u32 remaining = want;
@@ -1023,23 +1025,37 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     if (blockIdx.x == 0 && tid == 0) st->stamps[CWE_STAMPS - 1] = n_stamp;
 }
 
-int g_evict_grid = 0;
+// cw_score_evict_end: the victims of any deficit are a prefix of the (sorted) victims of the budget
+__global__ void evict_trim_kernel(const u32* deficit, u32 cap, const u32* n_budget, u32* num_victims, u32* status) {
+    const u32 want = min(*deficit, cap), have = *n_budget;  // have = min(cap, #evictable)
+    *num_victims = min(want, have);
+    if (have < want) atomicOr(status, CWS_CAPACITY);
+}
 
 }  // namespace
 
-int32_t cwi_score_evict(cw_ctx* ctx, u32 tick_now, u32 S, u32 F, const uint8_t* d_features, const int16_t* d_weights,
-                        i32 bias, const uint8_t* d_session_state, const u32* d_tau_override, const u32* d_deficit,
-                        u32 tier, u32* d_victims, u64* d_victim_scores, u32* d_num_victims, u32 cap) {
-    if (!g_evict_grid) {
-        CW_CUDA(ctx, cudaFuncSetAttribute(evict_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CWE_SMEM_BYTES));
-        int per_sm = 0;
-        CW_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, evict_kernel, CWE_THREADS, CWE_SMEM_BYTES));
-        if (per_sm < 1) {
-            snprintf(ctx->err, sizeof(ctx->err), "evict_kernel does not fit an SM");
-            return CW_E_CUDA;
-        }
-        g_evict_grid = ctx->n_sm;  // one CTA per SM: the cheapest grid barrier
+int32_t cwi_evict_init(cw_ctx* ctx) {
+    CW_CUDA(ctx, cudaFuncSetAttribute(evict_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CWE_SMEM_BYTES));
+    int per_sm = 0;
+    CW_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, evict_kernel, CWE_THREADS, CWE_SMEM_BYTES));
+    if (per_sm < 1) {
+        snprintf(ctx->err, sizeof(ctx->err), "evict_kernel does not fit an SM");
+        return CW_E_CUDA;
     }
+    ctx->evict_grid = ctx->n_sm;  // one CTA per SM: the cheapest grid barrier
+    return CW_OK;
+}
+
+int32_t cwi_evict_trim(cw_ctx* ctx, const u32* d_deficit, u32 cap, u32* d_num_victims) {
+    evict_trim_kernel<<<1, 1, 0, ctx->s_main>>>(d_deficit, cap, ctx->spec_n, d_num_victims, ctx->d_status);
+    CW_LAUNCH_CHECK(ctx);
+    return CW_OK;
+}
+
+int32_t cwi_score_evict(cw_ctx* ctx, cudaStream_t stream, u32 grid_limit, u32 tick_now, u32 S, u32 F,
+                        const uint8_t* d_features, const int16_t* d_weights, i32 bias, const uint8_t* d_session_state,
+                        const u32* d_tau_override, const u32* d_deficit, u32 tier, u32* d_victims, u64* d_victim_scores,
+                        u32* d_num_victims, u32 cap) {
     EvictArgs a;
     a.features = d_features;
     a.weights = d_weights;
@@ -1076,12 +1092,13 @@ int32_t cwi_score_evict(cw_ctx* ctx, u32 tick_now, u32 S, u32 F, const uint8_t* 
     a.num_victims = d_num_victims;
     // small pools do not need the whole machine (and the grid barrier gets cheaper)
     u32 tiles = (a.M + CWE_TILE - 1) / CWE_TILE;
-    int grid = g_evict_grid;
+    int grid = ctx->evict_grid;
+    if (grid_limit && (u32)grid > grid_limit) grid = (int)grid_limit;
     if ((u32)grid > tiles) grid = tiles ? (int)tiles : 1;
     // cooperative launch: the CTAs wait on one another at the grid barriers, so co-residency must be guaranteed
     void* kargs[] = {&a};
     CW_CUDA(ctx, cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(evict_kernel), dim3(grid), dim3(CWE_THREADS),
-                                             kargs, CWE_SMEM_BYTES, ctx->s_main));
+                                             kargs, CWE_SMEM_BYTES, stream));
     CW_LAUNCH_CHECK(ctx);
     return CW_OK;
 }

@@ -50,6 +50,7 @@ struct __align__(16) cw_slot {
 #define CW_KEY_EMPTY 0ull
 #define CW_KEY_TOMB 0xFFFFFFFFFFFFFFFFull
 #define CW_LOC_PENDING 0xFFFFFFFEu
+#define CWT_HIST_BINS 1024  // probe-length histogram of cw_table_stats (longer probes land in the last bin)
 
 __host__ __device__ __forceinline__ u64 cw_remap_key(u64 k) {
     if (k == CW_KEY_EMPTY) return 1ull;
@@ -115,6 +116,12 @@ struct cw_ctx {
     u64 n_slots;
     u32* ins_slot;   // scratch: slot index per input of an insert batch
     u32 ins_cap;
+    cw_slot* table2;  // second buffer of a compaction (allocated by the first one)
+    u32* tbl_cnt;     // device: [0] live keys, [1] tombstones, [2] longest probe of the last stats pass, [3] spare
+    u32* tbl_hist;    // device: probe-length histogram of cw_table_stats (CWT_HIST_BINS)
+    u64 live_ub;      // host upper bound of the live keys (exact after a refresh)
+    u64 tomb_ub;      // host upper bound of the tombstones created since the last compaction
+    u64 compactions;
     // metadata SoA, per tier
     u32* meta_session[2];
     u32* meta_last_access[2];
@@ -149,6 +156,14 @@ struct cw_ctx {
     u32* ev_bcur;    // scatter cursors (CWE_BUCKETS)
     u32* ev_blist;   // [0, 65536): medium buckets, [65536, 131072): large, [131072, 196608): non-empty
     u32 ev_cap;
+    int evict_grid;  // CTAs of the cooperative evict launch on THIS device (cw_create)
+    // stage 3, speculative form: side stream + fork / join events, victims of the budget, open flag
+    cudaStream_t s_side;
+    cudaEvent_t ev_fork, ev_spec;
+    u32* spec_n;     // device: victims the speculative selection produced (= min(cap, #evictable))
+    u32 spec_cap;
+    bool spec_open;
+    u32* dup_bits;   // CW_DEBUG: one bit per pool block (duplicate check of the gather)
     // stage 4
     uint8_t* staging;
     cudaEvent_t ev_gather[2], ev_copy[2], ev_join;
@@ -274,11 +289,18 @@ int32_t cwi_table_retag(cw_ctx*, const u64*, const u32*, u32);
 int32_t cwi_table_lookup(cw_ctx*, const u64*, u32, u32*);
 int32_t cwi_schedule(cw_ctx*, u32, const u32*, const u32*, const u64*, const u32*, u32, u32, u32, u32, u32*, u32*,
                      u32*);
-int32_t cwi_score_evict(cw_ctx*, u32, u32, u32, const uint8_t*, const int16_t*, i32, const uint8_t*, const u32*,
-                        const u32*, u32, u32*, u64*, u32*, u32);
+// stream: where the kernel runs; grid_limit: CTAs it may use (0 = one per SM); d_deficit == NULL: speculative
+// (deficit = cap, no capacity status, *d_num_victims = min(cap, #evictable))
+int32_t cwi_score_evict(cw_ctx*, cudaStream_t stream, u32 grid_limit, u32, u32, u32, const uint8_t*, const int16_t*, i32,
+                        const uint8_t*, const u32*, const u32*, u32, u32*, u64*, u32*, u32);
+int32_t cwi_evict_trim(cw_ctx*, const u32* d_deficit, u32 cap, u32* d_num_victims);
 int32_t cwi_copy_pages(cw_ctx*, cudaStream_t, const u32* d_ids, const u32* d_num, u32 first, u32 cap, void* d_staged,
                        bool gather);
 int32_t cwi_blocks_update(cw_ctx*, u32, const u32*, u32, const u32*, const u32*, const u32*, const u32*);
 int32_t cwi_predict_tau(cw_ctx*, u32, const u32*, const u32*, u32, const u64*, const u32*, u32*);
+int32_t cwi_table_compact(cw_ctx*);
+int32_t cwi_table_stats(cw_ctx*, u64* h_out8);
 int cwi_hash_grid(int n_sm);
 int cwi_copy_grid(int n_sm);
+int32_t cwi_evict_init(cw_ctx*);     // per-device function attributes + cooperative grid size (cw_create)
+int32_t cwi_schedule_init(cw_ctx*);  // per-device function attributes (cw_create)

@@ -365,6 +365,11 @@ __global__ void schedule_empty_kernel(u32* num_admit, u32* deficit) {
 
 }  // namespace
 
+int32_t cwi_schedule_init(cw_ctx* ctx) {
+    CW_CUDA(ctx, cudaFuncSetAttribute(schedule_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CWS_TILE * 8));
+    return CW_OK;
+}
+
 int32_t cwi_schedule(cw_ctx* ctx, u32 R, const u32* d_need, const u32* d_n_gpu, const u64* d_arrival_seq,
                      const u32* d_req_id, u32 policy, u32 free_blocks, u32 evictable, u32 max_admit, u32* d_order,
                      u32* d_num_admit, u32* d_deficit) {
@@ -376,11 +381,6 @@ int32_t cwi_schedule(cw_ctx* ctx, u32 R, const u32* d_need, const u32* d_n_gpu, 
     u32 ipc = (R + ctx->n_sm - 1) / ctx->n_sm;  // elements (warps) per CTA
     ipc = ipc < 8 ? 8 : ipc > CWS_MAX_I ? CWS_MAX_I : ipc;
     const u32 grid = (R + ipc - 1) / ipc;
-    static bool attr_set = false;
-    if (!attr_set) {
-        CW_CUDA(ctx, cudaFuncSetAttribute(schedule_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CWS_TILE * 8));
-        attr_set = true;
-    }
     size_t smem = (size_t)(R < CWS_TILE ? R : CWS_TILE) * 8;
     if (smem < 512) smem = 512;  // the fast path pads to 128 compressed keys
     schedule_kernel<<<grid, ipc * 32, smem, ctx->s_main>>>(R, d_need, d_n_gpu, d_arrival_seq, d_req_id, policy,

@@ -100,6 +100,24 @@ __global__ void __launch_bounds__(32) copy_pages_kernel(const CopyArgs a) {
     bulk_wait_all<0>();
 }
 
+#ifdef CW_DEBUG
+// debug builds: a block id that occurs twice in a gather list is a caller bug (SURVEY.md 8c stage 4)
+__global__ void dup_check_kernel(const u32* ids, const u32* num, u32 first, u32 cap, u32 pool_blocks, u32* bits,
+                                 u32* status, bool clear) {
+    u32 n = cap;
+    if (num) n = min(n, *num);
+    const u32 j = first + blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const u32 b = ids[j];
+    if (b >= pool_blocks) return;  // reported by the copy kernel itself
+    if (clear) {
+        bits[b >> 5] = 0;
+    } else if (atomicOr(&bits[b >> 5], 1u << (b & 31)) & (1u << (b & 31))) {
+        atomicOr(status, CWS_INVAL);
+    }
+}
+#endif
+
 }  // namespace
 
 int cwi_copy_grid(int n_sm) {
@@ -132,6 +150,13 @@ int32_t cwi_copy_pages(cw_ctx* ctx, cudaStream_t stream, const u32* d_ids, const
     a.pieces_per_chunk = (u32)((a.chunk_bytes + CWC_PIECE - 1) / CWC_PIECE);
     a.pool_blocks = ctx->cfg.num_blocks;
     a.status = ctx->d_status;
+#ifdef CW_DEBUG
+    if (gather && ctx->dup_bits) {
+        const u32 nb = (cap - first + 255) / 256;
+        dup_check_kernel<<<nb, 256, 0, stream>>>(d_ids, d_num, first, cap, a.pool_blocks, ctx->dup_bits, a.status, false);
+        dup_check_kernel<<<nb, 256, 0, stream>>>(d_ids, d_num, first, cap, a.pool_blocks, ctx->dup_bits, a.status, true);
+    }
+#endif
     const u64 items = (u64)(cap - first) * a.n_chunks * a.pieces_per_chunk;  // a.n_chunks: after coalescing
     u64 grid = (u64)ctx->copy_grid;
     if (grid > items) grid = items;

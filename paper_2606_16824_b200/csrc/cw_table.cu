@@ -12,6 +12,15 @@
 //   pass 3  the winners restore slot.idx = 0xFFFFFFFF
 // (All same-key threads follow one probe sequence whose slots only go from reusable to occupied during the
 // batch, so they converge on the same slot.)
+// A batch that could fill the table (live keys + batch > slots, decided on the host from an exact device counter)
+// is inserted by ONE thread in input order instead: which keys still find a slot is then the oracle's rule
+// (first come by input index), and the parallel path can never meet a full table.
+//
+// Erase leaves a TOMBSTONE (or EMPTY when the next slot is EMPTY: the cluster ends there, nothing can lie behind).
+// Tombstones are reclaimed by inserts that pass them and by COMPACTION: once the erases since the last compaction
+// could have turned a quarter of the slots into tombstones, the live entries are re-inserted into a second buffer
+// and copied back (the table address never changes, so captured graphs stay valid).  Every probe loop is bounded
+// by one full cycle: a table without EMPTY slots answers MISS for an absent key instead of spinning.
 //
 // Match: flat over hashes[]; a warp task is 128 consecutive hashes (one 32-ary search over hash_off for its first
 // request).  A task inside one request is probed LANE-INDEPENDENTLY: lane l owns hashes l + 32k, keys and results are
@@ -25,19 +34,13 @@
 // by this pass, and the table should own the L2.
 #include <stdio.h>
 
+#include <algorithm>
+
 #include "cw_internal.cuh"
 
 namespace {
 
-__device__ __forceinline__ uint4 ld_slot(const cw_slot* s) {
-#ifdef CW_SLOT_LDCG
-    return __ldcg(reinterpret_cast<const uint4*>(s));
-#elif defined(CW_SLOT_LDCV)
-    return __ldcv(reinterpret_cast<const uint4*>(s));
-#else
-    return *reinterpret_cast<const uint4*>(s);
-#endif
-}
+__device__ __forceinline__ uint4 ld_slot(const cw_slot* s) { return *reinterpret_cast<const uint4*>(s); }
 __device__ __forceinline__ u64 slot_key(const uint4& v) { return ((u64)v.y << 32) | v.x; }
 
 // returns slot index of `key` (already remapped) or ~0 if absent
@@ -82,12 +85,39 @@ __global__ void lookup_kernel(const cw_slot* table, u64 mask, const u64* keys, u
     loc[i] = l;
 }
 
-__global__ void erase_kernel(cw_slot* table, u64 mask, const u64* keys, u32 n) {
+// one counter update per warp: live keys, tombstones
+__device__ __forceinline__ void count_add(u32* cnt, bool live_up, bool live_down, bool tomb_up, bool tomb_down) {
+    const u32 lu = __popc(__ballot_sync(0xffffffffu, live_up)), ld = __popc(__ballot_sync(0xffffffffu, live_down));
+    const u32 tu = __popc(__ballot_sync(0xffffffffu, tomb_up)), td = __popc(__ballot_sync(0xffffffffu, tomb_down));
+    if ((threadIdx.x & 31) == 0) {
+        if (lu != ld) atomicAdd(&cnt[0], lu - ld);  // wraps for a negative difference: the sum stays exact
+        if (tu != td) atomicAdd(&cnt[1], tu - td);
+    }
+}
+
+__global__ void erase_kernel(cw_slot* table, u64 mask, const u64* keys, u32 n, u32* cnt) {
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    u32 l;
-    u64 s = table_find(table, mask, cw_remap_key(keys[i]), &l);
-    if (s != ~0ull) table[s].key = CW_KEY_TOMB;  // idx stays 0xFFFFFFFF, loc is dead
+    bool erased = false, tomb = false;
+    if (i < n) {
+        const u64 key = cw_remap_key(keys[i]);
+        u32 l;
+        u64 s = table_find(table, mask, key, &l);
+        if (s != ~0ull) {
+            // duplicates of a key inside the batch: exactly one thread wins the CAS and counts the erase
+            const u64 old = atomicCAS(reinterpret_cast<unsigned long long*>(&table[s].key), (unsigned long long)key,
+                                      (unsigned long long)CW_KEY_TOMB);  // idx stays 0xFFFFFFFF, loc is dead
+            if (old == key) {
+                erased = true;
+                // the cluster ends behind this slot: no probe sequence continues past it, so it can be EMPTY again
+                // (EMPTY slots never change during an erase batch; a neighbour erased concurrently is seen either as
+                // a key or as a tombstone -> this slot keeps its tombstone, which is still correct)
+                const u64 next = *reinterpret_cast<volatile unsigned long long*>(&table[(s + 1) & mask].key);
+                if (next == CW_KEY_EMPTY) *reinterpret_cast<volatile unsigned long long*>(&table[s].key) = CW_KEY_EMPTY;
+                else tomb = true;
+            }
+        }
+    }
+    count_add(cnt, false, erased, tomb, false);
 }
 
 __global__ void retag_kernel(cw_slot* table, u64 mask, const u64* keys, const u32* new_loc, u32 n) {
@@ -98,59 +128,153 @@ __global__ void retag_kernel(cw_slot* table, u64 mask, const u64* keys, const u3
     if (s != ~0ull) table[s].loc = new_loc[i];
 }
 
-__global__ void insert_claim_kernel(cw_slot* table, u64 mask, const u64* keys, u32 n, u32* ins_slot, u32* status) {
+__global__ void insert_claim_kernel(cw_slot* table, u64 mask, const u64* keys, u32 n, u32* ins_slot, u32* status,
+                                    u32* cnt) {
     u32 i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const u64 key = cw_remap_key(keys[i]);
-    const u64 home = key & mask;
-    u64 pos = home, steps = 0;
-    u64 found = ~0ull;
-    for (;;) {
-        // walk until the key, the end of the cluster (EMPTY) or a full cycle; remember the first reusable slot
-        u64 cand = ~0ull, cand_expect = 0;
-        while (steps <= mask) {
-            const u64 k = *reinterpret_cast<volatile unsigned long long*>(&table[pos].key);
+    bool claimed = false, from_tomb = false;
+    if (i < n) {
+        const u64 key = cw_remap_key(keys[i]);
+        const u64 home = key & mask;
+        u64 pos = home, steps = 0;
+        u64 found = ~0ull;
+        for (;;) {
+            // walk until the key, the end of the cluster (EMPTY) or a full cycle; remember the first reusable slot
+            u64 cand = ~0ull, cand_expect = 0;
+            while (steps <= mask) {
+                const u64 k = *reinterpret_cast<volatile unsigned long long*>(&table[pos].key);
+                if (k == key) {
+                    found = pos;
+                    break;
+                }
+                if (k == CW_KEY_TOMB && cand == ~0ull) {
+                    cand = pos;
+                    cand_expect = CW_KEY_TOMB;
+                }
+                if (k == CW_KEY_EMPTY) {
+                    if (cand == ~0ull) {
+                        cand = pos;
+                        cand_expect = CW_KEY_EMPTY;
+                    }
+                    break;
+                }
+                pos = (pos + 1) & mask;
+                ++steps;
+            }
+            if (found != ~0ull || cand == ~0ull) break;  // present, or table full
+            const u64 old = atomicCAS(reinterpret_cast<unsigned long long*>(&table[cand].key),
+                                      (unsigned long long)cand_expect, (unsigned long long)key);
+            if (old == cand_expect) {
+                table[cand].loc = CW_LOC_PENDING;
+                found = cand;
+                claimed = true;
+                from_tomb = cand_expect == CW_KEY_TOMB;
+                break;
+            }
+            if (old == key) {
+                found = cand;
+                break;
+            }
+            // another key took the slot: every slot before it is occupied by other keys for the rest of the
+            // batch, so the walk resumes there
+            pos = cand;
+            steps = (cand - home) & mask;
+        }
+        if (found != ~0ull) {
+            atomicMin(&table[found].idx, i);
+            ins_slot[i] = (u32)found;
+        } else {
+            ins_slot[i] = 0xFFFFFFFFu;
+            atomicOr(status, CWS_CAPACITY);
+        }
+    }
+    count_add(cnt, claimed, false, false, from_tomb);
+}
+
+// A batch that could fill the table: ONE thread inserts in input order, so the keys that still find a slot are the
+// first ones by input index (the oracle's rule; R2).  Misuse path (cw_create sizes the table for a load
+// factor <= 0.5): speed is irrelevant.
+__global__ void insert_seq_kernel(cw_slot* table, u64 mask, const u64* keys, const u32* loc, u32 n, u32* winner_loc,
+                                  u32* status, u32* cnt) {
+    if (blockIdx.x || threadIdx.x) return;
+    u32 live = cnt[0], tombs = cnt[1];
+    for (u32 i = 0; i < n; ++i) {
+        const u64 key = cw_remap_key(keys[i]);
+        u64 pos = key & mask, cand = ~0ull, found = ~0ull;
+        for (u64 steps = 0; steps <= mask; ++steps) {
+            const u64 k = table[pos].key;
             if (k == key) {
                 found = pos;
                 break;
             }
-            if (k == CW_KEY_TOMB && cand == ~0ull) {
-                cand = pos;
-                cand_expect = CW_KEY_TOMB;
-            }
+            if (k == CW_KEY_TOMB && cand == ~0ull) cand = pos;
             if (k == CW_KEY_EMPTY) {
-                if (cand == ~0ull) {
-                    cand = pos;
-                    cand_expect = CW_KEY_EMPTY;
-                }
+                if (cand == ~0ull) cand = pos;
                 break;
             }
             pos = (pos + 1) & mask;
-            ++steps;
         }
-        if (found != ~0ull || cand == ~0ull) break;  // present, or table full
-        const u64 old = atomicCAS(reinterpret_cast<unsigned long long*>(&table[cand].key),
-                                  (unsigned long long)cand_expect, (unsigned long long)key);
-        if (old == cand_expect) {
-            table[cand].loc = CW_LOC_PENDING;
-            found = cand;
-            break;
+        u32 w = CW_MISS;
+        if (found != ~0ull) {
+            w = table[found].loc;
+        } else if (cand != ~0ull) {
+            if (table[cand].key == CW_KEY_TOMB) --tombs;
+            ++live;
+            w = loc[i];
+            table[cand].key = key;
+            table[cand].loc = w;
+            table[cand].idx = 0xFFFFFFFFu;
+        } else {
+            atomicOr(status, CWS_CAPACITY);
         }
-        if (old == key) {
-            found = cand;
-            break;
-        }
-        // another key took the slot: every slot before it is occupied by other keys for the rest of the
-        // batch, so the walk resumes there
-        pos = cand;
-        steps = (cand - home) & mask;
+        if (winner_loc) winner_loc[i] = w;
     }
-    if (found != ~0ull) {
-        atomicMin(&table[found].idx, i);
-        ins_slot[i] = (u32)found;
-    } else {
-        ins_slot[i] = 0xFFFFFFFFu;
-        atomicOr(status, CWS_CAPACITY);
+    cnt[0] = live;
+    cnt[1] = tombs;
+}
+
+// Compaction: every live entry of `src` is re-inserted into the (cleared) second buffer; keys are unique, so one
+// CAS on the key decides the slot.
+__global__ void rebuild_kernel(const cw_slot* __restrict__ src, cw_slot* dst, u64 n_slots) {
+    const u64 mask = n_slots - 1;
+    for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n_slots; i += (u64)gridDim.x * blockDim.x) {
+        const uint4 v = ld_slot(src + i);
+        const u64 key = slot_key(v);
+        if (key == CW_KEY_EMPTY || key == CW_KEY_TOMB) continue;
+        u64 pos = key & mask;
+        for (u64 steps = 0; steps <= mask; ++steps) {
+            const u64 old = atomicCAS(reinterpret_cast<unsigned long long*>(&dst[pos].key),
+                                      (unsigned long long)CW_KEY_EMPTY, (unsigned long long)key);
+            if (old == CW_KEY_EMPTY) {
+                dst[pos].loc = v.z;
+                break;
+            }
+            pos = (pos + 1) & mask;
+        }
+    }
+}
+
+// cw_table_stats: exact recount of live keys / tombstones and the histogram of probe lengths (slots examined to
+// find each resident key = its distance from the home slot + 1).
+__global__ void stats_kernel(const cw_slot* __restrict__ table, u64 n_slots, u32* cnt, u32* hist) {
+    const u64 mask = n_slots - 1;
+    u32 live = 0, tombs = 0, longest = 0;
+    for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n_slots; i += (u64)gridDim.x * blockDim.x) {
+        const u64 key = slot_key(ld_slot(table + i));
+        if (key == CW_KEY_TOMB) ++tombs;
+        else if (key != CW_KEY_EMPTY) {
+            ++live;
+            const u64 d = ((i - (key & mask)) & mask) + 1;
+            longest = max(longest, (u32)min(d, (u64)0xFFFFFFFFull));
+            atomicAdd(&hist[min(d, (u64)CWT_HIST_BINS) - 1], 1u);
+        }
+    }
+    live = __reduce_add_sync(0xffffffffu, live);
+    tombs = __reduce_add_sync(0xffffffffu, tombs);
+    longest = __reduce_max_sync(0xffffffffu, longest);
+    if ((threadIdx.x & 31) == 0) {
+        if (live) atomicAdd(&cnt[0], live);
+        if (tombs) atomicAdd(&cnt[1], tombs);
+        if (longest) atomicMax(&cnt[2], longest);
     }
 }
 
@@ -181,9 +305,7 @@ __global__ void insert_reset_kernel(cw_slot* table, u32 n, const u32* ins_slot) 
 // ---------------------------------------------------------------------------------------------- match
 // full occupancy (<= 32 registers, 2048 threads per SM): the probe is bound by resident warps x latency (93 us vs 107 us
 // at 6 CTAs/SM on configs[2])
-#ifndef MATCH_THREADS
 #define MATCH_THREADS 64  // measured on configs[2]: 256 -> 66.1 us, 128 -> 65.9, 64 -> 64.6 (CTA slots turn over per 2 tasks)
-#endif
 #define MATCH_MIN_CTAS (2048 / MATCH_THREADS)
 #define CWM_CHUNK 128  // consecutive hashes handled by one warp task (4 rounds of 32): measured optimum on configs[2]
                        // (64: 89 us, 128: 75, 256: 79, 512: ~85, 1024: ~100, 2048: ~170 — long tasks are bound by the
@@ -264,8 +386,9 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
                                  : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
                                  : "l"(table + slot));
                     const bool hit = v.x == key.x && v.y == key.y;
-                    const bool empty = (v.x | v.y) == 0;
                     slot = (slot + 1) & mask;
+                    // EMPTY ends the cluster; so does a full cycle (a table without EMPTY slots must not spin)
+                    const bool empty = (v.x | v.y) == 0 || (!hit && slot == (key.x & mask));
                     if (hit || empty) {  // resolved: record, next key of this lane
                         wloc[pos] = hit ? v.z : CW_MISS;
                         if (empty) miss_at = pos;
@@ -362,6 +485,7 @@ __global__ void __launch_bounds__(256) match_finish_kernel(const u64* __restrict
     const u32 lane = threadIdx.x & 31;
     const u32 r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     if (r >= R) return;
+    if (hash_off[R] - hash_off[0] > 0xFFFFFFFFull) return;  // rejected by the probe kernel: outputs untouched
     const u64 h0 = hash_off[r];
     const u32 n_r = (u32)(hash_off[r + 1] - h0);
     const u32 k = min(first_miss[r], n_r);
@@ -415,10 +539,72 @@ int32_t cwi_table_lookup(cw_ctx* ctx, const u64* d_keys, u32 n, u32* d_loc) {
     CW_LAUNCH_CHECK(ctx);
     return CW_OK;
 }
+static bool stream_capturing(cudaStream_t s) {
+    cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(s, &st) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return st != cudaStreamCaptureStatusNone;
+}
+
+int32_t cwi_table_compact(cw_ctx* ctx) {
+    const size_t bytes = ctx->n_slots * sizeof(cw_slot);
+    if (!ctx->table2) CW_CUDA(ctx, cudaMalloc(reinterpret_cast<void**>(&ctx->table2), bytes));
+    cudaStream_t s = ctx->s_main;
+    CW_CUDA(ctx, cudaMemsetAsync(ctx->table2, 0, bytes, s));
+    CW_CUDA(ctx, cudaMemset2DAsync(reinterpret_cast<uint8_t*>(ctx->table2) + 12, sizeof(cw_slot), 0xFF, 4, ctx->n_slots, s));
+    const u32 grid = (u32)std::min<u64>((ctx->n_slots + 255) / 256, (u64)ctx->n_sm * 16);
+    rebuild_kernel<<<grid, 256, 0, s>>>(ctx->table, ctx->table2, ctx->n_slots);
+    CW_LAUNCH_CHECK(ctx);
+    // copied back: the table address is baked into captured graphs and must not change
+    CW_CUDA(ctx, cudaMemcpyAsync(ctx->table, ctx->table2, bytes, cudaMemcpyDeviceToDevice, s));
+    CW_CUDA(ctx, cudaMemsetAsync(ctx->tbl_cnt + 1, 0, sizeof(u32), s));
+    ctx->tomb_ub = 0;
+    ctx->compactions++;
+    return CW_OK;
+}
+
+int32_t cwi_table_stats(cw_ctx* ctx, u64* h_out8) {
+    cudaStream_t s = ctx->s_main;
+    CW_CUDA(ctx, cudaMemsetAsync(ctx->tbl_cnt, 0, 4 * sizeof(u32), s));
+    CW_CUDA(ctx, cudaMemsetAsync(ctx->tbl_hist, 0, CWT_HIST_BINS * sizeof(u32), s));
+    const u32 grid = (u32)std::min<u64>((ctx->n_slots + 255) / 256, (u64)ctx->n_sm * 16);
+    stats_kernel<<<grid, 256, 0, s>>>(ctx->table, ctx->n_slots, ctx->tbl_cnt, ctx->tbl_hist);
+    CW_LAUNCH_CHECK(ctx);
+    u32 cnt[4];
+    static thread_local u32 hist[CWT_HIST_BINS];
+    CW_CUDA(ctx, cudaMemcpyAsync(cnt, ctx->tbl_cnt, sizeof(cnt), cudaMemcpyDeviceToHost, s));
+    CW_CUDA(ctx, cudaMemcpyAsync(hist, ctx->tbl_hist, sizeof(hist), cudaMemcpyDeviceToHost, s));
+    CW_CUDA(ctx, cudaStreamSynchronize(s));
+    ctx->live_ub = cnt[0];  // exact again
+    u64 sum = 0, p50 = 0, p99 = 0, acc = 0;
+    for (u32 b = 0; b < CWT_HIST_BINS; ++b) sum += (u64)hist[b] * (b + 1);  // the last bin counts its lower edge
+    for (u32 b = 0; b < CWT_HIST_BINS; ++b) {
+        acc += hist[b];
+        if (!p50 && cnt[0] && acc * 2 >= cnt[0]) p50 = b + 1;
+        if (!p99 && cnt[0] && acc * 100 >= (u64)cnt[0] * 99) p99 = b + 1;
+    }
+    h_out8[0] = cnt[0];
+    h_out8[1] = cnt[1];
+    h_out8[2] = ctx->n_slots;
+    h_out8[3] = cnt[2];
+    h_out8[4] = p50;
+    h_out8[5] = p99;
+    h_out8[6] = ctx->compactions;
+    h_out8[7] = sum;
+    return CW_OK;
+}
+
 int32_t cwi_table_erase(cw_ctx* ctx, const u64* d_keys, u32 n) {
     if (!n) return CW_OK;
-    erase_kernel<<<cdiv(n, 256), 256, 0, ctx->s_main>>>(ctx->table, ctx->n_slots - 1, d_keys, n);
+    erase_kernel<<<cdiv(n, 256), 256, 0, ctx->s_main>>>(ctx->table, ctx->n_slots - 1, d_keys, n, ctx->tbl_cnt);
     CW_LAUNCH_CHECK(ctx);
+    // tombstones are bounded from the host (no read-back): once the erases since the last compaction could have
+    // turned a quarter of the slots into tombstones, rebuild (never inside a graph capture: the launch sequence of
+    // a captured call must not depend on the table's history)
+    ctx->tomb_ub += n;
+    if (ctx->tomb_ub > ctx->n_slots / 4 && !stream_capturing(ctx->s_main)) return cwi_table_compact(ctx);
     return CW_OK;
 }
 int32_t cwi_table_retag(cw_ctx* ctx, const u64* d_keys, const u32* d_new_loc, u32 n) {
@@ -429,6 +615,26 @@ int32_t cwi_table_retag(cw_ctx* ctx, const u64* d_keys, const u32* d_new_loc, u3
 }
 int32_t cwi_table_insert(cw_ctx* ctx, const u64* d_keys, const u32* d_loc, u32 n, u32* d_winner_loc) {
     if (!n) return CW_OK;
+    const u64 mask = ctx->n_slots - 1;
+    if (ctx->live_ub + n > ctx->n_slots) {
+        // the batch might fill the table: replace the host bound by the exact device count (one sync, misuse path)
+        if (stream_capturing(ctx->s_main)) {
+            snprintf(ctx->err, sizeof(ctx->err), "cw_table_insert near a full table cannot be captured");
+            return CW_E_STATE;
+        }
+        u32 live = 0;
+        CW_CUDA(ctx, cudaMemcpyAsync(&live, ctx->tbl_cnt, sizeof(u32), cudaMemcpyDeviceToHost, ctx->s_main));
+        CW_CUDA(ctx, cudaStreamSynchronize(ctx->s_main));
+        ctx->live_ub = live;
+    }
+    if (ctx->live_ub + n > ctx->n_slots) {  // first come by input index, like the oracle
+        insert_seq_kernel<<<1, 32, 0, ctx->s_main>>>(ctx->table, mask, d_keys, d_loc, n, d_winner_loc, ctx->d_status,
+                                                     ctx->tbl_cnt);
+        CW_LAUNCH_CHECK(ctx);
+        ctx->live_ub = ctx->n_slots;
+        return CW_OK;
+    }
+    ctx->live_ub += n;
     if (n > ctx->ins_cap) {  // grow the per-batch scratch (outside of graph capture)
         if (ctx->ins_slot) CW_CUDA(ctx, cudaFree(ctx->ins_slot));
         ctx->ins_slot = nullptr;
@@ -436,9 +642,8 @@ int32_t cwi_table_insert(cw_ctx* ctx, const u64* d_keys, const u32* d_loc, u32 n
         CW_CUDA(ctx, cudaMalloc(&ctx->ins_slot, (size_t)n * sizeof(u32)));
         ctx->ins_cap = n;
     }
-    const u64 mask = ctx->n_slots - 1;
     insert_claim_kernel<<<cdiv(n, 256), 256, 0, ctx->s_main>>>(ctx->table, mask, d_keys, n, ctx->ins_slot,
-                                                               ctx->d_status);
+                                                               ctx->d_status, ctx->tbl_cnt);
     CW_LAUNCH_CHECK(ctx);
     insert_resolve_kernel<<<cdiv(n, 256), 256, 0, ctx->s_main>>>(ctx->table, d_loc, n, ctx->ins_slot, d_winner_loc);
     CW_LAUNCH_CHECK(ctx);

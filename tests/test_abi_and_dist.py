@@ -20,6 +20,7 @@ HEADER = os.path.join(ROOT, "include", "cachewise.h")
 def _declared():
     src = open(HEADER).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    src = re.sub(r"#ifdef CW_DEBUG.*?#endif", "", src, flags=re.S)  # debug-build-only diagnostics
     return sorted(set(re.findall(r"\b(cw_[a-z_0-9]+)\s*\(", src)))
 
 

@@ -280,7 +280,7 @@ def test_swap_out_swap_in_round_trip_through_pinned_host(layout):
     # (b) slot-addressed host tier, some slots consecutive (coalesced copies) and some not
     slots = np.array([5, 6, 7, 30, 2, 3, 40, 41, 42, 43, 0, 20, 21, 9, 11, 10, 50, 51, 52, 1], np.uint32)
     tier = torch.zeros(64 * page, dtype=torch.uint8).pin_memory()
-    ctx.swap_out(dev(vic), dev(np.array([n], np.uint32)), n, slots, tier)
+    ctx.swap_out(dev(vic), None, n, slots, tier)
     assert ctx.sync(check=False) == 0
     exp_tier = oracle.swap_out(pool_np, n_chunks, chunk_bytes, cfg["chunk_stride"], cfg["block_stride"], vic,
                                np.zeros(64 * page, np.uint8), slots=slots)

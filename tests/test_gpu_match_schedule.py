@@ -56,11 +56,13 @@ def test_table_insert_erase_retag_semantics():
     ot.retag([5, 9], [HOST | 3, 77])
     assert (_lookup(ctx, q) == ot.lookup(q)).all()
     win, _ = _insert(ctx, [9], [91])  # tombstone reuse
+    ot.insert([9], [91])
     assert win.tolist() == [91] and _lookup(ctx, [9]).tolist() == [91]
-    # capacity: 16 slots, 5 live -> 11 of 20 new keys fit; which ones is unspecified on the GPU
+    # capacity: 16 slots, 5 live -> the FIRST 11 of 20 new keys (by input index) fit, as in the oracle
     keys = np.arange(1000, 1020, dtype=np.uint64)
     win, st = _insert(ctx, keys, np.arange(20, dtype=np.uint32))
-    assert st == -2 and (win != MISS).sum() == 11
+    ewin, est = ot.insert(keys, np.arange(20, dtype=np.uint32))
+    assert st == est == -2 and (win == ewin).all() and (win != MISS).sum() == 11
     got = _lookup(ctx, keys)
     assert (got == win).all()
     ctx.close()

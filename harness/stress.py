@@ -54,13 +54,14 @@ class StressStep:
     def __init__(self, snap: gen.StressSnapshot, stream: torch.cuda.Stream, with_pool: bool = True,
                  layout: str = "block", n_chunks: int = STEP_N_CHUNKS, chunk_bytes: int = STEP_CHUNK_BYTES,
                  staging_bytes: int = 128 << 20, policy: int = cw.POLICY_MIN_ADDITIONAL, free_blocks: int = 0,
-                 holes: bool = False, new_requests: int = 256):
+                 holes: bool = False, new_requests: int = 256, spec_ctas: int = 0):
         self.snap, self.stream = snap, stream
         S, L = snap.streams.shape
         self.S, self.L, self.RB, self.M = S, L, snap.resident_blocks, snap.M
         self.R = snap.tok_off.size - 1
         self.F = snap.features.shape[1]
         self.policy, self.free_blocks = policy, free_blocks
+        self.spec_ctas = spec_ctas                # CTAs of the speculative selection (0 = library default)
         self.evict_budget = snap.deficit          # "eviction deficit 5% of the pool per step"
         self.cap = max(snap.deficit, 1)
         self.page = n_chunks * chunk_bytes
@@ -151,12 +152,30 @@ class StressStep:
     def scatter(self):
         self.ctx.scatter_pages(self.d_vic, self.d_nv, self.cap, self.d_staged)
 
-    def decide(self, steady: bool = False):
-        """Stages 1-3 (the <=100 us target of BASELINE.json)."""
+    def score_evict_begin(self):
+        s = self.snap
+        self.ctx.score_evict_begin(s.tick_now, self.S, self.F, self.d_feat, self.d_w, s.bias, self.d_state, None, 0,
+                                   self.d_vic, self.d_sc, self.cap, self.spec_ctas)
+
+    def score_evict_end(self):
+        self.ctx.score_evict_end(self.d_def, self.d_nv)
+
+    def decide(self, steady: bool = False, overlap: bool = True):
+        """Stages 1-3 (the <=100 us target of BASELINE.json).  overlap: the selection of the eviction budget runs on
+        the ctx's side stream beside hash -> match -> schedule (cw_score_evict_begin / _end); otherwise the four
+        calls run in series."""
+        # a cold step hashes 421 MB of token ids and wants every SM for it: the fork comes after the hash there
+        if overlap and steady:
+            self.score_evict_begin()
         self.hash(steady)
+        if overlap and not steady:
+            self.score_evict_begin()
         self.match()
         self.schedule()
-        self.score_evict()
+        if overlap:
+            self.score_evict_end()
+        else:
+            self.score_evict()
 
     def step(self, steady: bool = False):
         """One pass of the whole hot path with everything resident in HBM (device halves of stage 4)."""

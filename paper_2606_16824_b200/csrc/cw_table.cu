@@ -366,9 +366,11 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
             u32* wloc = s_loc[threadIdx.x >> 5];
             {
                 u64 kk[KPL];
+                // UNCONDITIONAL loads at clamped positions: a predicated load followed by its own use is not hoisted by
+                // the compiler, and the four loads then complete one after the other
 #pragma unroll
                 for (int q = 0; q < KPL; ++q)  // in flight together; streaming (evict-first): the table stays in L2
-                    kk[q] = lane + 32 * q < n_task ? __ldcs(hs + c0 + lane + 32 * q) : 0;
+                    kk[q] = __ldcs(hs + c0 + min(lane + 32 * q, n_task - 1));
 #pragma unroll
                 for (int q = 0; q < KPL; ++q) wkey[lane + 32 * q] = cw_remap_key(kk[q]);  // read back by this lane only
             }

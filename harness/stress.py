@@ -54,7 +54,7 @@ class StressStep:
     def __init__(self, snap: gen.StressSnapshot, stream: torch.cuda.Stream, with_pool: bool = True,
                  layout: str = "block", n_chunks: int = STEP_N_CHUNKS, chunk_bytes: int = STEP_CHUNK_BYTES,
                  staging_bytes: int = 128 << 20, policy: int = cw.POLICY_MIN_ADDITIONAL, free_blocks: int = 0,
-                 holes: bool = False, new_requests: int = 256, spec_ctas: int = 0):
+                 holes: bool = False, new_requests: int = 256, spec_ctas: int = 0, stream_copy=None):
         self.snap, self.stream = snap, stream
         S, L = snap.streams.shape
         self.S, self.L, self.RB, self.M = S, L, snap.resident_blocks, snap.M
@@ -86,7 +86,7 @@ class StressStep:
             self.n_chunks, self.chunk_bytes = n_chunks, chunk_bytes
             self.ctx = cw.Context(num_blocks=self.M, table_log2_slots=snap.table_log2, max_requests=max(self.R, S),
                                   max_hashed_blocks=max(self.n_hashed, S * (L // 16), 1), max_sessions=S,
-                                  max_features=16, stream_main=stream, **kw)
+                                  max_features=16, stream_main=stream, stream_copy=stream_copy, **kw)
             c = self.ctx
             # resident set: blocks [0,RB) of every session stream, hashed by the CUDA path itself
             d_stream = dev(np.concatenate([snap.streams.reshape(-1), np.zeros(4, np.int32)]))
@@ -117,6 +117,7 @@ class StressStep:
             self.d_order = torch.zeros(R, **i32)
             self.d_na, self.d_def, self.d_nv = torch.zeros(1, **i32), torch.zeros(1, **i32), torch.zeros(1, **i32)
             self.d_vic = torch.zeros(self.cap, **i32)
+            self.d_vic_prev = torch.zeros(self.cap, **i32)   # victims whose pages are still on their way back
             self.d_sc = torch.zeros(self.cap, dtype=torch.int64, device="cuda")
             self.d_staged = torch.empty(self.cap * self.page, dtype=torch.uint8, device="cuda") if with_pool else None
             # steady state: hashes persist, only the last `new_requests` requests of the queue are new arrivals

@@ -358,3 +358,69 @@ def test_out_of_range_block_id_is_reported_and_touches_nothing():
     ctx.gather_pages(dev(np.array([3, 8], np.uint32)), None, 2, staged)
     assert ctx.sync(check=False) == -1
     ctx.close()
+
+
+def _c3_words(b, c, n_words, n_chunks):
+    """Procedural content of chunk c of block b as uint64 words (harness arithmetic: a counter through a mixer)."""
+    base = (np.asarray(b, np.uint64).reshape(-1, 1) * np.uint64(n_chunks) + np.uint64(c)) * np.uint64(n_words)
+    with np.errstate(over="ignore"):
+        w = (base + np.arange(n_words, dtype=np.uint64).reshape(1, -1)) * np.uint64(0xD6E8FEB86659FD93)
+        w ^= w >> np.uint64(29)
+    return w
+
+
+def test_swap_config3_shape_llama70b_pages_layer_major_60gib_pool():
+    """BASELINE.json configs[3] at its own shape: 160 chunks x 32 KiB = 5 MiB pages scattered over a 60 GiB
+    LAYER-MAJOR pool (12,288 blocks); 512 random victims gathered to pinned host and restored into 512 other blocks.
+    cw_swap_out / cw_swap_in against cwo_swap_out / cwo_swap_in, every byte of every page; the oracle's 60 GiB pool is
+    a lazily mapped zero array in which only the blocks the test touches are filled."""
+    import torch
+    from gpu_util import dev
+    torch.cuda.empty_cache()
+    if torch.cuda.mem_get_info()[0] < 70 << 30:
+        pytest.skip("needs 70 GiB of free HBM")
+    n_chunks, chunk, M, n = 160, 32768, 12288, 512
+    page, n_words = n_chunks * chunk, chunk // 8
+    cs, bs = M * chunk, chunk
+    pool = torch.empty(M * page, dtype=torch.uint8, device="cuda")
+    pv = pool.view(torch.int64).view(n_chunks, M, n_words)
+    wi = torch.arange(n_words, dtype=torch.int64, device="cuda").unsqueeze(0)
+    bi = torch.arange(M, dtype=torch.int64, device="cuda").unsqueeze(1)
+    for c in range(n_chunks):                                    # the same words as _c3_words, computed by torch
+        w = ((bi * n_chunks + c) * n_words + wi) * (-2960836687051489901)   # 0xD6E8FEB86659FD93 as int64
+        w ^= (w >> 29) & ((1 << 35) - 1)
+        pv[c] = w
+    ctx = __import__("paper_2606_16824_b200").Context(
+        num_blocks=M, table_log2_slots=15, max_requests=1, max_hashed_blocks=1, n_chunks=n_chunks, chunk_bytes=chunk,
+        chunk_stride=cs, block_stride=bs, pool=pool, staging_bytes=2 * (320 << 20))
+    g = gen.rng(35, 0)
+    perm = g.permutation(M)
+    vic, dst, bystanders = perm[:n].astype(np.uint32), perm[n:2 * n].astype(np.uint32), perm[2 * n:2 * n + 64]
+    # the oracle's pool: 60 GiB of lazily mapped zeros, filled only where the test looks
+    opool = np.zeros(M * page, np.uint8)
+    ov = opool.view(np.uint64).reshape(n_chunks, M, n_words)
+    touched = np.concatenate([vic, dst, bystanders.astype(np.uint32)])
+    for c in range(n_chunks):
+        ov[c, touched] = _c3_words(touched, c, n_words, n_chunks)
+    # ---- swap-out
+    h = torch.zeros(n * page, dtype=torch.uint8).pin_memory()
+    ctx.swap_out(dev(vic), None, n, None, h)
+    assert ctx.sync(check=False) == 0
+    exp = oracle.swap_out(opool, n_chunks, chunk, cs, bs, vic, np.zeros(n * page, np.uint8))
+    assert np.array_equal(h.numpy(), exp), "swap-out bytes (512 x 5 MiB pages)"
+    # ---- the device-count form (TMA stores straight to pinned host) at the same shape
+    h2 = torch.zeros(64 * page, dtype=torch.uint8).pin_memory()
+    ctx.swap_out(dev(vic), dev(np.array([37], np.uint32)), 64, None, h2)
+    assert ctx.sync(check=False) == 0
+    assert np.array_equal(h2.numpy()[:37 * page], exp[:37 * page]) and not h2.numpy()[37 * page:].any()
+    # ---- swap-in into other blocks
+    ctx.swap_in(None, h, dev(dst), n)
+    assert ctx.sync(check=False) == 0
+    oracle.swap_in(opool, n_chunks, chunk, cs, bs, exp, dst)
+    look = np.concatenate([dst.astype(np.int64), vic.astype(np.int64), bystanders.astype(np.int64)])
+    got = pool.view(n_chunks, M, chunk)[:, torch.from_numpy(look).cuda(), :].cpu().numpy()
+    want = opool.reshape(n_chunks, M, chunk)[:, look, :]
+    assert np.array_equal(got, want), "pool bytes after swap-in (destinations, sources and bystanders)"
+    ctx.close()
+    del pool, pv
+    torch.cuda.empty_cache()

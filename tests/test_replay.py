@@ -140,24 +140,48 @@ def test_gpu_long_agent_replay_reduced():
     gb.close()
 
 
-@pytest.mark.gpu
-@pytest.mark.parametrize("which", [1, 4])
-def test_gpu_full_size_replay_counts(which):
-    """BASELINE.json configs[1] / configs[4] at full session and turn counts (pools capped by the box, scale
-    stated in the note).  Minutes of wall clock and terabytes over PCIe: runs only when CW_FULL_REPLAY_<which> is
-    set to a divisor of the session count (1 = full)."""
+def _full_size_replay(which, scale):
+    """BASELINE.json configs[1] / configs[4] page shapes and trace recipes through the shared driver on both backends:
+    every step's hashes, overlaps, order, admission, victims + scores, host drops and counts must be identical, KV
+    bytes of sampled victims are checked against the procedural page content, and the table's probe lengths are
+    reported (tombstone compaction keeps them short over millions of erases)."""
     import json
     import os
-    scale = int(os.environ.get(f"CW_FULL_REPLAY_{which}", "0"))
-    if scale < 1:
-        pytest.skip(f"set CW_FULL_REPLAY_{which}=1 (or a divisor) to run the full-size replay")
+
+    import torch
+    torch.cuda.empty_cache()
     tr, cfg, note = replay.full_config(which, scale=scale)
     ro, rg, gb = _both(tr, cfg, len(tr.sessions), tr.F, verify_pages=1)
     diffs = replay.compare(ro, rg)
+    stats = gb.ctx.table_stats()
     out = dict(config=cfg.name, note=note, oracle=ro.totals(), gpu=rg.totals(), pages_verified=gb.pages_verified,
-               differences=len(diffs))
+               differences=len(diffs), table=stats)
     os.makedirs("gpurun_out", exist_ok=True)
     with open(f"gpurun_out/replay_full_config{which}.json", "w") as f:
         json.dump(out, f)
     gb.close()
-    assert diffs == [] and ro.totals() == rg.totals() and rg.evictions > 0
+    torch.cuda.empty_cache()
+    assert diffs == [] and ro.totals() == rg.totals() and rg.evictions > 0 and gb.pages_verified > 0
+    assert stats["probe_p99"] <= 64 and stats["tombstones"] <= stats["slots"] // 2, stats
+    return out
+
+
+@pytest.mark.gpu
+def test_gpu_replay_config1_full_size_64_sessions_x_40_turns():
+    """BASELINE.json configs[1] at FULL size: 64 sessions x 40 turns, 2 MiB layer-major pages, pool = 60% of the
+    working set capped at 120 GiB of HBM, host tier capped at 48 GiB pinned (the caps are stated in the note written
+    to gpurun_out/).  About four minutes, most of it the CPU oracle."""
+    out = _full_size_replay(1, 1)
+    assert out["gpu"]["completed"] == 64 * 40
+
+
+@pytest.mark.gpu
+def test_gpu_replay_config4_quarter_scale_128_sessions_x_50_turns():
+    """BASELINE.json configs[4] at 1/4 of its session and turn counts (128 sessions x 50 turns, contexts growing to
+    200k tokens, 896 KiB pages, 130,789-block pool, 48 GiB pinned host tier): the largest scale whose two replays
+    (oracle + CUDA) fit in about ten minutes.  CW_FULL_REPLAY_4=2 or =1 runs the 1/2-scale (about an hour) or the full
+    trace instead."""
+    import os
+    scale = int(os.environ.get("CW_FULL_REPLAY_4", "4"))
+    out = _full_size_replay(4, scale)
+    assert out["gpu"]["completed"] == (512 // scale) * (200 // scale)

@@ -521,10 +521,15 @@ def run_cuda(args):
                 h_scal[1:2].copy_(st.d_def, non_blocking=True)
                 h_scal[2:3].copy_(st.d_nv, non_blocking=True)
                 stream.synchronize()
-                upload(k ^ 1)                          # next step's token ids: overlaps this step's swap-out
                 n = int(h_scal[2])
+                # results first: a read-back queued behind the 15 ms swap-out would hold the main stream for that long
+                h_order.copy_(st.d_order, non_blocking=True)
+                h_k.copy_(st.d_k, non_blocking=True)
+                h_g.copy_(st.d_g, non_blocking=True)
+                h_vic[:n].copy_(st.d_vic[:n], non_blocking=True)
                 if pending[0]:
                     st.ctx.swap_in(None, h_swap, st.d_vic_prev, pending[0])   # H2D queued behind the previous D2H
+                upload(k ^ 1)                          # next step's token ids: H2D beside this step's swap-out D2H
                 st.d_vic_prev[:n].copy_(st.d_vic[:n], non_blocking=True)
                 if mark:
                     tl["out0"] = torch.cuda.Event(enable_timing=True)
@@ -536,10 +541,6 @@ def run_cuda(args):
                     tl["d2h1"] = torch.cuda.Event(enable_timing=True)
                     tl["d2h1"].record(copy_stream)     # behind the last device->host copy
                 pending[0] = n
-                h_order.copy_(st.d_order, non_blocking=True)
-                h_k.copy_(st.d_k, non_blocking=True)
-                h_g.copy_(st.d_g, non_blocking=True)
-                h_vic[:n].copy_(st.d_vic[:n], non_blocking=True)
                 return n
 
             Ke = max(3, min(K, 20))

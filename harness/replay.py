@@ -43,6 +43,10 @@ class ReplayConfig:
     c0_ms: int = 20                 # integer service model: c0 + ceil(c_tok*new_tokens/1000) + c_blk*swapped_in
     c_tok_us: int = 250
     c_blk_ms: int = 1
+    token_budget: int = 0           # chunked prefill (512 tokens per chunk): new tokens an engine
+                                    # iteration may prefill; admission goes through cw_admit_chunked; 0 = unlimited
+    offload: str = "swap"           # service cost of a host-tier hit: "swap" = PCIe swap-in (c_blk_ms per
+                                    # block), "auto" = the cheaper of swap-in and recomputing those 16 tokens per block
     store_bytes: bool = True        # log the staged bytes of every swap-out (tiny configs only)
     max_steps: int = 1_000_000
 
@@ -84,6 +88,7 @@ class StepLog:
     host_drops: np.ndarray
     staged: np.ndarray
     swapped_in: int
+    chunk: np.ndarray = None        # cw_admit_chunked: tokens each queued request may prefill this iteration
 
 
 @dataclass
@@ -97,11 +102,26 @@ class ReplayResult:
     completed: int = 0
     end_ms: int = 0
     session_done_ms: dict = field(default_factory=dict)
+    page_bytes: int = 0
+    swap_outs: int = 0              # pages that physically crossed PCIe device -> host
+    prefill_iterations: int = 0     # engine iterations spent on prefill chunks (token_budget > 0)
+    new_tokens: int = 0             # tokens prefilled (token goodput numerator)
 
     def totals(self):
         return dict(steps=len(self.steps), evictions=self.evictions, drops=self.drops, swap_ins=self.swap_ins,
                     hit_blocks=self.hit_blocks, new_blocks=self.new_blocks, completed=self.completed,
                     end_ms=self.end_ms)
+
+    def metrics(self):
+        """The paper's session-level metrics (PAPER.md 6.1 L287, 6.4 L337) in the replay's virtual time."""
+        done = list(self.session_done_ms.values())
+        return dict(
+            transfer_volume_bytes=self.evictions * self.page_bytes,          # L337: eviction count x KV block size
+            pcie_bytes=(self.swap_outs + self.swap_ins) * self.page_bytes,   # what the offload tier really moved (L345)
+            mean_session_ms=int(np.mean(done)) if done else 0,               # L287 (3): request latencies, no tool time
+            token_goodput_per_s=round(self.new_tokens * 1000.0 / max(self.end_ms, 1), 1),     # L287 (1)
+            requests_per_s=round(self.completed * 1000.0 / max(self.end_ms, 1), 3),
+            prefill_iterations=self.prefill_iterations)
 
 
 def tail_tag(session: int, turn: int) -> int:
@@ -122,7 +142,7 @@ def lcp_blocks(a: np.ndarray, b: np.ndarray) -> int:
 def run(trace: gen.Trace, cfg: ReplayConfig, be) -> ReplayResult:
     """Replays `trace` against backend `be`.  Deterministic given the backend's answers."""
     S, F, M, HS = len(trace.sessions), trace.F, cfg.num_blocks, cfg.host_slots
-    res = ReplayResult()
+    res = ReplayResult(page_bytes=cfg.page)
     free_hbm = list(range(M))
     free_host = list(range(HS))
     heapq.heapify(free_hbm)
@@ -207,6 +227,11 @@ def run(trace: gen.Trace, cfg: ReplayConfig, be) -> ReplayResult:
         order, num_admit, deficit = be.schedule(need, n_gpu, np.array([q.arrival_seq for q in queue], np.uint64),
                                                 np.array([q.req_id for q in queue], np.uint32), cfg.policy,
                                                 len(free_hbm), evictable, cfg.max_admit)
+        chunk = None
+        if cfg.token_budget:   # chunked prefill: the iteration's token budget bounds the admitted prefix (L271)
+            new_tok = np.array([q.tokens.size - 16 * int(k_total[i]) for i, q in enumerate(queue)], np.uint32)
+            chunk, num_admit, deficit = be.admit_chunked(order, need, n_gpu, new_tok, len(free_hbm), evictable,
+                                                         cfg.max_admit, cfg.token_budget)
         # ---- 5. pin + touch the hits of the admitted requests (a request whose own hits use up the evictable
         #         blocks it was counting on stays queued)
         admitted, need_sum, pinned = [], 0, 0
@@ -273,6 +298,7 @@ def run(trace: gen.Trace, cfg: ReplayConfig, be) -> ReplayResult:
             if vs.size:
                 slots = np.array([heapq.heappop(free_host) for _ in range(vs.size)], np.uint32)
                 staged = be.swap_out(vs, slots, cfg.store_bytes, b_hash[vs])
+                res.swap_outs += int(vs.size)
                 be.table_retag(b_hash[vs], slots | np.uint32(HOST_BIT))
                 h_hash[slots], h_sess[slots], h_depth[slots], h_last[slots] = b_hash[vs], b_sess[vs], b_depth[vs], b_last[vs]
                 h_valid[slots] = True
@@ -337,7 +363,14 @@ def run(trace: gen.Trace, cfg: ReplayConfig, be) -> ReplayResult:
                 res.new_blocks += n_new
             res.hit_blocks += k
             new_tokens = q.tokens.size - 16 * k
-            svc = cfg.c0_ms + (cfg.c_tok_us * new_tokens + 999) // 1000 + cfg.c_blk_ms * int(host.size)
+            res.new_tokens += new_tokens
+            # chunked prefill: the request occupies ceil(new_tokens / budget) engine iterations of c0 each
+            iters = max(1, -(-new_tokens // cfg.token_budget)) if cfg.token_budget else 1
+            res.prefill_iterations += iters
+            swap_ms = cfg.c_blk_ms * int(host.size)
+            if cfg.offload == "auto":   # L345: PCIe swap-in vs recomputing the same blocks, whichever is cheaper
+                swap_ms = min(swap_ms, (cfg.c_tok_us * 16 * int(host.size) + 999) // 1000)
+            svc = cfg.c0_ms * iters + (cfg.c_tok_us * new_tokens + 999) // 1000 + swap_ms
             svc_max = max(svc_max, svc)
             done_reqs.append((q, shared, private))
         res.swap_ins += swapped_in
@@ -379,7 +412,7 @@ def run(trace: gen.Trace, cfg: ReplayConfig, be) -> ReplayResult:
             gone.add(q.req_id)
         res.steps.append(StepLog(step, now, [q.req_id for q in queue], new_hashes, k_total, n_gpu, order, num_admit,
                                  deficit, [q.req_id for q, _, _ in done_reqs], victims, vscores, host_drops, staged,
-                                 swapped_in))
+                                 swapped_in, chunk if chunk is not None else np.zeros(0, np.uint32)))
         queue = [q for q in queue if q.req_id not in gone]
         tick += 1
     res.end_ms = now
@@ -406,7 +439,7 @@ def policy_sweep(trace: gen.Trace, base: ReplayConfig, make_backend):
         cfg = dataclasses.replace(base, policy=sched, evict_policy=ev, use_hint=False)
         r = run(trace, cfg, make_backend(cfg))
         t = r.totals()
-        t["mean_session_ms"] = int(np.mean(list(r.session_done_ms.values())))
+        t.update(r.metrics())
         out[name] = t
     return out
 
@@ -416,11 +449,13 @@ def compare(a: ReplayResult, b: ReplayResult):
     diffs = []
     if a.totals() != b.totals():
         diffs.append(("totals", a.totals(), b.totals()))
+    if a.metrics() != b.metrics():
+        diffs.append(("metrics", a.metrics(), b.metrics()))
     for x, y in zip(a.steps, b.steps):
         for f in ("now_ms", "queued", "num_admit", "deficit", "admitted", "swapped_in"):
             if getattr(x, f) != getattr(y, f):
                 diffs.append((x.step, f, getattr(x, f), getattr(y, f)))
-        for f in ("new_hashes", "k_total", "n_gpu", "order", "victims", "victim_scores", "host_drops", "staged"):
+        for f in ("new_hashes", "k_total", "n_gpu", "order", "victims", "victim_scores", "host_drops", "staged", "chunk"):
             u, v = getattr(x, f), getattr(y, f)
             if u.shape != v.shape or not np.array_equal(u, v):
                 diffs.append((x.step, f, u.shape, v.shape))
@@ -489,6 +524,18 @@ class GpuBackend:
             self.ctx.sync()
             sc = self.st.host(d_s, np.uint32)
             return self.st.host(d_o, np.uint32)[:R], int(sc[0]), int(sc[1])
+
+    def admit_chunked(self, order, need, n_gpu, new_tokens, free, evictable, max_admit, token_budget):
+        t, R = self.torch, need.size
+        with t.cuda.stream(self.stream):
+            d_c = t.zeros(max(R, 1), dtype=t.int32, device="cuda")
+            d_s = t.zeros(2, dtype=t.int32, device="cuda")
+            self.ctx.admit_chunked(R, self._dev(order, np.uint32), self._dev(need), self._dev(n_gpu),
+                                   self._dev(new_tokens, np.uint32), free, evictable, max_admit, token_budget, d_c,
+                                   d_s[0:1], d_s[1:2])
+            self.ctx.sync()
+            sc = self.st.host(d_s, np.uint32)
+            return self.st.host(d_c, np.uint32)[:R].copy(), int(sc[0]), int(sc[1])
 
     def blocks_update(self, tier, ids, session=None, depth=None, last_access=None, ref_flags=None):
         if ids.size == 0:

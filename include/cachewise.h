@@ -134,6 +134,19 @@ int32_t cw_schedule(cw_ctx* ctx, uint32_t R, const uint32_t* d_need, const uint3
                     uint32_t free_blocks, uint32_t evictable, uint32_t max_admit, uint32_t* d_order,
                     uint32_t* d_num_admit, uint32_t* d_deficit);
 
+/* NEXT-3 — admission under a chunked-prefill token budget (PAPER.md 6.1 L271 "chunked-prefill enabled
+ * ... max. 512 tokens per chunk"; reading R8: an engine iteration prefills at most token_budget new tokens).
+ * Re-runs the admission walk of cw_schedule over its output d_order: request i (a_i = max(d_i - n_gpu_i, 0) more
+ * blocks, d_new_tokens[i] tokens to prefill) is admitted while count < max_admit, need + a_i <= free_blocks +
+ * evictable and tokens handed out so far < token_budget; it receives min(d_new_tokens[i], budget left).  Stops at the
+ * first request that does not fit.
+ *   d_chunk_tokens uint32[R], by INPUT index: tokens each request may prefill this iteration (0 = not admitted, or
+ *   nothing to prefill); d_num_admit / d_deficit as in cw_schedule.  d_order[p] >= R -> CW_E_INVAL at cw_sync. */
+int32_t cw_admit_chunked(cw_ctx* ctx, uint32_t R, const uint32_t* d_order, const uint32_t* d_need,
+                         const uint32_t* d_n_gpu, const uint32_t* d_new_tokens, uint32_t free_blocks,
+                         uint32_t evictable, uint32_t max_admit, uint64_t token_budget, uint32_t* d_chunk_tokens,
+                         uint32_t* d_num_admit, uint32_t* d_deficit);
+
 /* Stage 3 — reuse-aware eviction (PAPER.md 5.2 L215-219 evict in decreasing predicted time-to-next-reuse,
  * L181 j* = argmax_{j != i} tau_j, L252 unreferenced blocks only and one prediction per session, L277 idle
  * sessions first, L281 LRU fallback).  DESIGN.md reading R4.
@@ -165,8 +178,8 @@ int32_t cw_score_evict(cw_ctx* ctx, uint32_t tick_now, uint32_t S, uint32_t F, c
  * the output arrays must not be touched between begin and end.  One begin may be outstanding per ctx (a second one,
  * or an end without a begin, returns CW_E_STATE).  Both calls can be captured into one CUDA graph on stream_main (the
  * side stream joins the capture as a parallel branch).
- *   n_ctas: how many CTAs (= SMs) the speculative kernel may occupy; 0 = library default (a quarter of the SMs, so
- *   that the kernels on stream_main keep the rest of the machine). */
+ *   n_ctas: how many CTAs (= SMs) the speculative kernel may occupy; 0 = library default (3/8 of the SMs: measured
+ *   on configs[2], 56 of 148 CTAs is where neither branch of the step waits for the other). */
 int32_t cw_score_evict_begin(cw_ctx* ctx, uint32_t tick_now, uint32_t S, uint32_t F, const uint8_t* d_features,
                              const int16_t* d_weights, int32_t bias, const uint8_t* d_session_state,
                              const uint32_t* d_tau_override, uint32_t tier, uint32_t* d_victims,

@@ -151,6 +151,21 @@ def schedule(need_d, n_gpu, arrival_seq, req_id, policy, free_blocks, evictable,
     return order, na.value, de.value
 
 
+def admit_chunked(order, need_d, n_gpu, new_tokens, free_blocks, evictable, max_admit, token_budget):
+    """PAPER.md L271 chunked prefill (R8).  Returns (chunk_tokens[R] by input index, num_admit, deficit)."""
+    order, need_d, n_gpu = _arr(order, np.uint32), _arr(need_d, np.uint32), _arr(n_gpu, np.uint32)
+    new_tokens = _arr(new_tokens, np.uint32)
+    R = need_d.size
+    chunk = np.zeros(R, np.uint32)
+    na, de = C.c_uint32(0), C.c_uint32(0)
+    st = lib().cwo_admit_chunked(C.c_uint32(R), _p(order), _p(need_d), _p(n_gpu), _p(new_tokens),
+                                 C.c_uint32(free_blocks), C.c_uint32(evictable), C.c_uint32(max_admit),
+                                 C.c_uint64(token_budget), _p(chunk), C.byref(na), C.byref(de))
+    if st:
+        raise ValueError(f"cwo_admit_chunked status {st}")
+    return chunk, na.value, de.value
+
+
 def session_tau(features, weights, bias, session_state, tau_override=None):
     features = _arr(features, np.uint8)
     S, F = features.shape

@@ -39,6 +39,9 @@ class OracleBackend:
     def schedule(self, need, n_gpu, arr, rid, policy, free, evictable, max_admit):
         return oracle.schedule(need, n_gpu, arr, rid, policy, free, evictable, max_admit)
 
+    def admit_chunked(self, order, need, n_gpu, new_tokens, free, evictable, max_admit, token_budget):
+        return oracle.admit_chunked(order, need, n_gpu, new_tokens, free, evictable, max_admit, token_budget)
+
     def blocks_update(self, tier, ids, session=None, depth=None, last_access=None, ref_flags=None):
         m = self.meta[tier]
         for name, v in (("session", session), ("depth", depth), ("last_access", last_access), ("ref_flags", ref_flags)):

@@ -222,6 +222,35 @@ int cwo_schedule(u32 R, const u32* need_d, const u32* n_gpu, const u64* arrival_
     return 0;
 }
 
+// NEXT-3 — admission under a chunked-prefill token budget.  PAPER.md 6.1 L271: "All experiments run
+// with chunked-prefill enabled and we use the default value of max. 512 tokens per chunk".  DESIGN.md reading R8: an
+// engine iteration prefills at most `token_budget` new tokens.  Walk the dispatch order of cwo_schedule; request i
+// (needing a_i = d_i - k_i more blocks and t_i new tokens) is admitted while count < max_admit, the blocks fit
+// (need + a_i <= free + evictable, L177) and budget is left (used < token_budget); it gets the chunk
+// min(t_i, token_budget - used).  Stop at the first request that does not fit (no back-filling).  chunk_tokens is in
+// INPUT-index order, 0 for everybody who was not admitted; deficit = max(0, need - free_blocks) as in cwo_schedule.
+int cwo_admit_chunked(u32 R, const u32* order, const u32* need_d, const u32* n_gpu, const u32* new_tokens,
+                      u32 free_blocks, u32 evictable, u32 max_admit, u64 token_budget, u32* chunk_tokens,
+                      u32* num_admit, u32* deficit) {
+    for (u32 i = 0; i < R; ++i) chunk_tokens[i] = 0;
+    u64 need = 0, used = 0, budget = (u64)free_blocks + (u64)evictable;
+    u32 count = 0;
+    for (u32 p = 0; p < R; ++p) {
+        u32 i = order[p];
+        if (i >= R) return -1;
+        u64 a = need_d[i] > n_gpu[i] ? (u64)(need_d[i] - n_gpu[i]) : 0;
+        if (count >= max_admit || need + a > budget || used >= token_budget) break;
+        u64 chunk = std::min<u64>(new_tokens[i], token_budget - used);
+        chunk_tokens[i] = (u32)chunk;
+        used += chunk;
+        need += a;
+        ++count;
+    }
+    *num_admit = count;
+    *deficit = need > free_blocks ? (u32)std::min<u64>(need - free_blocks, 0xFFFFFFFFull) : 0;
+    return 0;
+}
+
 // ------------------------------------------------------------------------------------------------
 // Stage 3 — reuse-aware eviction.  PAPER.md 5.2 L215-219 (evict in decreasing tau; Belady with true
 // tau), L181 (j* = argmax_{j != i} tau_j), L252 (unreferenced blocks only; one prediction per

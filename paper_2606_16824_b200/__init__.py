@@ -24,7 +24,7 @@ CW_REF_PINNED = 0x40000000
 POLICY_MIN_ADDITIONAL, POLICY_OVERLAP_FIRST, POLICY_FCFS = 0, 1, 2
 
 EXPORTS = ["cw_create", "cw_destroy", "cw_sync", "cw_join_copy", "cw_last_error", "cw_launch_count", "cw_hash_blocks",
-           "cw_match_prefix", "cw_schedule", "cw_score_evict", "cw_score_evict_begin", "cw_score_evict_end",
+           "cw_match_prefix", "cw_schedule", "cw_admit_chunked", "cw_score_evict", "cw_score_evict_begin", "cw_score_evict_end",
            "cw_predict_tau", "cw_swap_out", "cw_swap_in", "cw_gather_pages", "cw_scatter_pages", "cw_table_insert",
            "cw_table_erase", "cw_table_retag", "cw_table_lookup", "cw_table_compact", "cw_table_stats",
            "cw_blocks_update"]
@@ -72,6 +72,7 @@ def lib():
         L.cw_hash_blocks.argtypes = [P, P, P, P, P, P, P, U32, P]
         L.cw_match_prefix.argtypes = [P, P, P, U32, P, P, P]
         L.cw_schedule.argtypes = [P, U32, P, P, P, P, U32, U32, U32, U32, P, P, P]
+        L.cw_admit_chunked.argtypes = [P, U32, P, P, P, P, U32, U32, U32, U64, P, P, P]
         L.cw_score_evict.argtypes = [P, U32, U32, U32, P, P, I32, P, P, P, U32, P, P, P, U32]
         L.cw_score_evict_begin.argtypes = [P, U32, U32, U32, P, P, I32, P, P, U32, P, P, U32, U32]
         L.cw_score_evict_end.argtypes = [P, P, P]
@@ -177,6 +178,12 @@ class Context:
         self._ck(lib().cw_schedule(self._h, R, _ptr(need), _ptr(n_gpu), _ptr(arrival_seq), _ptr(req_id), policy,
                                    free_blocks, evictable, max_admit, _ptr(order), _ptr(num_admit), _ptr(deficit)),
                  "cw_schedule")
+
+    def admit_chunked(self, R, order, need, n_gpu, new_tokens, free_blocks, evictable, max_admit, token_budget,
+                      chunk_tokens, num_admit, deficit):
+        self._ck(lib().cw_admit_chunked(self._h, R, _ptr(order), _ptr(need), _ptr(n_gpu), _ptr(new_tokens), free_blocks,
+                                        evictable, max_admit, token_budget, _ptr(chunk_tokens), _ptr(num_admit),
+                                        _ptr(deficit)), "cw_admit_chunked")
 
     def score_evict(self, tick_now, S, F, features, weights, bias, session_state, tau_override, deficit, tier, victims,
                     victim_scores, num_victims, cap):

@@ -260,6 +260,17 @@ int32_t cw_schedule(cw_ctx* ctx, uint32_t R, const uint32_t* d_need, const uint3
                         d_order, d_num_admit, d_deficit);
 }
 
+int32_t cw_admit_chunked(cw_ctx* ctx, uint32_t R, const uint32_t* d_order, const uint32_t* d_need,
+                         const uint32_t* d_n_gpu, const uint32_t* d_new_tokens, uint32_t free_blocks,
+                         uint32_t evictable, uint32_t max_admit, uint64_t token_budget, uint32_t* d_chunk_tokens,
+                         uint32_t* d_num_admit, uint32_t* d_deficit) {
+    if (!ctx) return CW_E_STATE;
+    if (!d_num_admit || !d_deficit || R > ctx->cfg.max_requests) return CW_E_INVAL;
+    if (R && (!d_order || !d_need || !d_n_gpu || !d_new_tokens || !d_chunk_tokens)) return CW_E_INVAL;
+    return cwi_admit_chunked(ctx, R, d_order, d_need, d_n_gpu, d_new_tokens, free_blocks, evictable, max_admit,
+                             token_budget, d_chunk_tokens, d_num_admit, d_deficit);
+}
+
 static int32_t check_evict_args(cw_ctx* ctx, uint32_t S, uint32_t F, const uint8_t* d_features,
                                 const int16_t* d_weights, int32_t bias, const uint8_t* d_session_state,
                                 const uint32_t* d_tau_override, uint32_t tier, const uint32_t* d_victims) {

@@ -293,6 +293,8 @@ int32_t cwi_schedule(cw_ctx*, u32, const u32*, const u32*, const u64*, const u32
 // (deficit = cap, no capacity status, *d_num_victims = min(cap, #evictable))
 int32_t cwi_score_evict(cw_ctx*, cudaStream_t stream, u32 grid_limit, u32, u32, u32, const uint8_t*, const int16_t*, i32,
                         const uint8_t*, const u32*, const u32*, u32, u32*, u64*, u32*, u32);
+int32_t cwi_admit_chunked(cw_ctx*, u32, const u32*, const u32*, const u32*, const u32*, u32, u32, u32, u64, u32*, u32*,
+                          u32*);
 int32_t cwi_evict_trim(cw_ctx*, const u32* d_deficit, u32 cap, u32* d_num_victims);
 int32_t cwi_copy_pages(cw_ctx*, cudaStream_t, const u32* d_ids, const u32* d_num, u32 first, u32 cap, void* d_staged,
                        bool gather);

@@ -358,6 +358,100 @@ __global__ void __launch_bounds__(CWA_THREADS)
     }
 }
 
+// NEXT-3: admission under a chunked-prefill token budget (PAPER.md 6.1 L271, R8).  Both
+// running sums (blocks, tokens) only grow along the dispatch order, so "admitted" is a prefix of it and every test of
+// the sequential walk becomes a test on exclusive / inclusive prefix sums: one CTA, two 64-bit block scans.
+__global__ void __launch_bounds__(CWA_THREADS)
+    admit_chunked_kernel(u32 R, const u32* __restrict__ order, const u32* __restrict__ need, const u32* __restrict__ n_gpu,
+                         const u32* __restrict__ new_tokens, u32 free_blocks, u32 evictable, u32 max_admit,
+                         u64 token_budget, u32* chunk_tokens, u32* num_admit, u32* deficit, u32* status) {
+    __shared__ u64 s_a[CWA_THREADS / 32], s_t[CWA_THREADS / 32];
+    __shared__ u32 s_count;
+    __shared__ unsigned long long s_need;
+    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) {
+        s_count = 0;
+        s_need = 0;
+    }
+    const u32 per = (R + CWA_THREADS - 1) / CWA_THREADS;
+    const u32 lo = min(R, tid * per), hi = min(R, lo + per);
+    u64 sum_a = 0, sum_t = 0;
+    bool bad = false;
+    for (u32 p = lo; p < hi; ++p) {
+        const u32 i = order[p];
+        if (i >= R) {
+            bad = true;
+            continue;
+        }
+        const u32 d = need[i], g = n_gpu[i];
+        sum_a += d > g ? d - g : 0;
+        sum_t += new_tokens[i];
+    }
+    if (bad) atomicOr(status, CWS_INVAL);
+    u64 inc_a = sum_a, inc_t = sum_t;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const u64 ya = shfl64_up(inc_a, d), yt = shfl64_up(inc_t, d);
+        if (lane >= (u32)d) {
+            inc_a += ya;
+            inc_t += yt;
+        }
+    }
+    if (lane == 31) {
+        s_a[warp] = inc_a;
+        s_t[warp] = inc_t;
+    }
+    __syncthreads();
+    if (warp == 0) {
+        const u64 wa = s_a[lane], wt = s_t[lane];
+        u64 ia = wa, it = wt;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const u64 ya = shfl64_up(ia, d), yt = shfl64_up(it, d);
+            if (lane >= (u32)d) {
+                ia += ya;
+                it += yt;
+            }
+        }
+        s_a[lane] = ia - wa;  // exclusive
+        s_t[lane] = it - wt;
+    }
+    __syncthreads();
+    u64 run_a = s_a[warp] + inc_a - sum_a, run_t = s_t[warp] + inc_t - sum_t;  // sums over everything before `lo`
+    const u64 budget = (u64)free_blocks + (u64)evictable;
+    u32 cnt = 0;
+    u64 last_need = 0;
+    for (u32 p = lo; p < hi; ++p) {
+        const u32 i = order[p];
+        if (i >= R) continue;
+        const u32 d = need[i], g = n_gpu[i];
+        const u64 a = d > g ? d - g : 0, t = new_tokens[i];
+        const bool in = p < max_admit && run_a + a <= budget && run_t < token_budget;  // monotone in p
+        u32 chunk = 0;
+        if (in) {
+            chunk = (u32)min(t, token_budget - run_t);
+            ++cnt;
+            last_need = run_a + a;
+        }
+        chunk_tokens[i] = chunk;
+        run_a += a;
+        run_t += t;
+    }
+    const u32 wc = __reduce_add_sync(0xffffffffu, cnt);
+    const u32 nh = __reduce_max_sync(0xffffffffu, (u32)(last_need >> 32));
+    const u32 nl = __reduce_max_sync(0xffffffffu, (u32)(last_need >> 32) == nh ? (u32)last_need : 0u);
+    if (lane == 0 && wc) {
+        atomicAdd(&s_count, wc);
+        atomicMax(&s_need, ((unsigned long long)nh << 32) | nl);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        *num_admit = s_count;
+        const u64 nd = s_need;
+        *deficit = nd > free_blocks ? (u32)min(nd - free_blocks, (u64)0xFFFFFFFFull) : 0u;
+    }
+}
+
 __global__ void schedule_empty_kernel(u32* num_admit, u32* deficit) {
     *num_admit = 0;
     *deficit = 0;
@@ -388,6 +482,21 @@ int32_t cwi_schedule(cw_ctx* ctx, u32 R, const u32* d_need, const u32* d_n_gpu, 
     CW_LAUNCH_CHECK(ctx);
     admit_kernel<<<1, CWA_THREADS, 0, ctx->s_main>>>(R, ctx->sched_a, free_blocks, evictable, max_admit, d_num_admit,
                                                      d_deficit);
+    CW_LAUNCH_CHECK(ctx);
+    return CW_OK;
+}
+
+int32_t cwi_admit_chunked(cw_ctx* ctx, u32 R, const u32* d_order, const u32* d_need, const u32* d_n_gpu,
+                          const u32* d_new_tokens, u32 free_blocks, u32 evictable, u32 max_admit, u64 token_budget,
+                          u32* d_chunk_tokens, u32* d_num_admit, u32* d_deficit) {
+    if (R == 0) {
+        schedule_empty_kernel<<<1, 1, 0, ctx->s_main>>>(d_num_admit, d_deficit);
+        CW_LAUNCH_CHECK(ctx);
+        return CW_OK;
+    }
+    admit_chunked_kernel<<<1, CWA_THREADS, 0, ctx->s_main>>>(R, d_order, d_need, d_n_gpu, d_new_tokens, free_blocks,
+                                                             evictable, max_admit, token_budget, d_chunk_tokens,
+                                                             d_num_admit, d_deficit, ctx->d_status);
     CW_LAUNCH_CHECK(ctx);
     return CW_OK;
 }

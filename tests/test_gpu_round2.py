@@ -299,3 +299,41 @@ def test_debug_build_rejects_duplicate_victims(tmp_path):
     out = subprocess.run([sys.executable, str(script)], env=dict(os.environ, CACHEWISE_DEBUG="1"), capture_output=True,
                          text=True, timeout=600)
     assert out.returncode == 0 and "debug ok" in out.stdout, out.stdout + out.stderr
+
+
+# ---------------------------------------------------------------------------------------------- NEXT-3: chunked prefill
+@pytest.mark.parametrize("R", [1, 2, 33, 1025, 5000])
+def test_admit_chunked_matches_the_oracle(R):
+    """PAPER.md L271 (chunked prefill, 512 tokens per chunk) as an admission budget: cw_schedule -> cw_admit_chunked
+    against cwo_schedule -> cwo_admit_chunked, every output, budgets from 0 to unlimited, both block regimes."""
+    from gpu_util import dev, host, small_ctx, zeros
+    g = gen.rng(78, R)
+    ctx = small_ctx(max_requests=max(R, 8))
+    need = g.integers(1, 3000, size=R).astype(np.uint32)
+    n_gpu = np.minimum(need, g.integers(0, 3000, size=R)).astype(np.uint32)
+    n_gpu[::7] = need[::7]                                                  # full hits: nothing to prefill
+    new_tok = ((need - n_gpu).astype(np.int64) * 16 - g.integers(0, 16, size=R)).clip(0).astype(np.uint32)
+    arr, rid = g.permutation(R).astype(np.uint64), np.arange(R, dtype=np.uint32)
+    d_need, d_g, d_t = dev(need), dev(n_gpu), dev(new_tok)
+    d_order, d_na, d_de = zeros(R, np.uint32), zeros(1, np.uint32), zeros(1, np.uint32)
+    d_chunk = zeros(R, np.uint32)
+    for policy in (0, 1, 2):
+        for free, evictable in ((0, 50_000), (1_000, 4_000_000_000), (7, 0)):
+            ctx.schedule(R, d_need, d_g, dev(arr), dev(rid), policy, free, evictable, R, d_order, d_na, d_de)
+            eorder, _, _ = oracle.schedule(need, n_gpu, arr, rid, policy, free, evictable, R)
+            for budget in (0, 1, 512, 8192, (1 << 32) + 5, (1 << 63)):
+                for max_admit in (1, 8, R):
+                    d_chunk.fill_(-1)
+                    ctx.admit_chunked(R, d_order, d_need, d_g, d_t, free, evictable, max_admit, budget, d_chunk, d_na,
+                                      d_de)
+                    assert ctx.sync(check=False) == 0
+                    ech, ena, ede = oracle.admit_chunked(eorder, need, n_gpu, new_tok, free, evictable, max_admit, budget)
+                    assert host(d_order, np.uint32)[:R].tolist() == eorder.tolist()
+                    assert host(d_chunk, np.uint32)[:R].tolist() == ech.tolist(), (policy, free, budget, max_admit)
+                    assert (int(host(d_na, np.uint32)[0]), int(host(d_de, np.uint32)[0])) == (ena, ede)
+    # a corrupt order is reported, not followed
+    bad = np.arange(R, dtype=np.uint32)
+    bad[0] = R + 3
+    ctx.admit_chunked(R, dev(bad), d_need, d_g, d_t, 0, 10, R, 512, d_chunk, d_na, d_de)
+    assert ctx.sync(check=False) == -1
+    ctx.close()

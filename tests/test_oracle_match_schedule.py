@@ -165,3 +165,47 @@ def test_schedule_special_cases():
     d = np.array([5, 9, 1], np.uint32)
     o, na, de = oracle.schedule(d, np.zeros(3, np.uint32), [0, 1, 2], [0, 1, 2], 2, 4, 6, 3)
     assert o.tolist() == [0, 1, 2] and na == 1 and de == 1
+
+
+# ---------------------------------------------------------------------------------------------- NEXT-3: chunked prefill
+def _admit_chunked_brute(order, need, n_gpu, new_tokens, free, evictable, max_admit, budget):
+    """PAPER.md L271 / DESIGN.md R8 restated as the literal loop, in Python integers."""
+    chunk = [0] * len(need)
+    used = blocks = count = 0
+    for i in order:
+        a = max(int(need[i]) - int(n_gpu[i]), 0)
+        if count >= max_admit or blocks + a > free + evictable or used >= budget:
+            break
+        chunk[i] = min(int(new_tokens[i]), budget - used)
+        used += chunk[i]
+        blocks += a
+        count += 1
+    return chunk, count, max(0, blocks - free)
+
+
+def test_admit_chunked_matches_the_literal_loop_and_its_special_cases():
+    g = gen.rng(77, 0)
+    for R in (1, 2, 17, 300):
+        need = g.integers(1, 400, size=R).astype(np.uint32)
+        n_gpu = np.minimum(need, g.integers(0, 400, size=R)).astype(np.uint32)
+        new_tok = ((need - n_gpu).astype(np.int64) * 16 - g.integers(0, 16, size=R)).clip(0).astype(np.uint32)
+        arr, rid = g.permutation(R).astype(np.uint64), np.arange(R, dtype=np.uint32)
+        for policy in (0, 2):
+            order, na0, de0 = oracle.schedule(need, n_gpu, arr, rid, policy, 50, 3000, R)
+            for budget in (0, 1, 512, 2048, 10**7, 1 << 40):
+                for max_admit in (1, 5, R):
+                    ch, na, de = oracle.admit_chunked(order, need, n_gpu, new_tok, 50, 3000, max_admit, budget)
+                    ech, ena, ede = _admit_chunked_brute(order, need, n_gpu, new_tok, 50, 3000, max_admit, budget)
+                    assert ch.tolist() == ech and (na, de) == (ena, ede), (R, policy, budget, max_admit)
+                    # invariants: the budget is never exceeded; only the LAST admitted request can get a partial chunk
+                    assert int(ch.sum()) <= budget or budget == 0
+                    adm = [int(i) for i in order[:na]]
+                    assert all(ch[i] == new_tok[i] for i in adm[:-1])
+                    assert all(ch[int(i)] == 0 for i in order[na:])
+            # an unlimited budget admits exactly what cwo_schedule admits
+            ch, na, de = oracle.admit_chunked(order, need, n_gpu, new_tok, 50, 3000, R, 1 << 62)
+            assert (na, de) == (na0, de0) and (ch[order[:na]] == new_tok[order[:na]]).all()
+    # requests with nothing to prefill (full hits) cost no budget and do not stop the walk
+    order = np.arange(4, dtype=np.uint32)
+    ch, na, de = oracle.admit_chunked(order, [5, 5, 5, 5], [5, 5, 1, 0], [0, 0, 600, 80], 0, 100, 4, 512)
+    assert ch.tolist() == [0, 0, 512, 0] and na == 3 and de == 4     # the 4th finds the budget used up

@@ -88,6 +88,39 @@ def test_comparison_systems_reproduce_the_shape_of_the_papers_gains():
     assert res["CacheWise (prefix-aware + predictor)"]["mean_session_ms"] < res["vLLM (FCFS + LRU)"]["mean_session_ms"]
 
 
+def test_chunked_prefill_budget_transfer_volume_and_offload_cost_model():
+    """SURVEY.md 8f NEXT-3.  (a) L271: a 512-token chunk budget admits fewer requests per iteration and every request
+    then occupies ceil(new_tokens / 512) iterations, so sessions take longer, while WHAT is computed is unchanged;
+    (b) L337: transfer volume = evictions x page size, and the PCIe bytes of the offload tier = (swap-outs +
+    swap-ins) x page size; (c) L345: with offload="auto" a host hit costs the cheaper of swap-in and recompute, so
+    it can only shorten the service time, and it does when PCIe is made slower than prefill."""
+    tr = gen.tiny_trace(0)
+    base = tiny_cfg(num_blocks=160, host_slots=48)
+    r0 = replay.run(tr, base, OracleBackend(base, 4, 4))
+    cfg = tiny_cfg(num_blocks=160, host_slots=48, token_budget=512)
+    r1 = replay.run(tr, cfg, OracleBackend(cfg, 4, 4))
+    assert r0.completed == r1.completed == 32
+    assert r1.hit_blocks + r1.new_blocks == r0.hit_blocks + r0.new_blocks
+    assert r1.prefill_iterations > r1.completed >= r0.prefill_iterations == r0.completed
+    assert r1.metrics()["mean_session_ms"] > r0.metrics()["mean_session_ms"]   # tool gaps dominate end_ms itself
+    for st in r1.steps:   # at most 512 tokens handed out per iteration; only admitted requests get a chunk
+        assert int(st.chunk.sum()) <= 512 and np.count_nonzero(st.chunk) <= st.num_admit
+    for r in (r0, r1):
+        m = r.metrics()
+        assert m["transfer_volume_bytes"] == r.evictions * base.page and r.evictions > 0
+        assert m["pcie_bytes"] == (r.swap_outs + r.swap_ins) * base.page and r.swap_outs == r.evictions - (r.drops - _host_drops(r))
+        assert m["token_goodput_per_s"] > 0 and m["mean_session_ms"] > 0
+    slow_pcie = dict(num_blocks=160, host_slots=48, c_blk_ms=50)
+    ra = replay.run(tr, tiny_cfg(**slow_pcie), OracleBackend(tiny_cfg(**slow_pcie), 4, 4))
+    rb = replay.run(tr, tiny_cfg(offload="auto", **slow_pcie), OracleBackend(tiny_cfg(offload="auto", **slow_pcie), 4, 4))
+    assert ra.swap_ins > 0 and rb.metrics()["mean_session_ms"] < ra.metrics()["mean_session_ms"]
+
+
+def _host_drops(r):
+    """Host-tier entries dropped to make room (they were evicted from HBM earlier; not HBM evictions themselves)."""
+    return sum(int(s.host_drops.size) for s in r.steps)
+
+
 # ---------------------------------------------------------------------------------------------- GPU parity
 def _both(tr, cfg, S, F, verify_pages=0):
     ro = replay.run(tr, cfg, OracleBackend(cfg, S, F))
@@ -100,7 +133,8 @@ def _both(tr, cfg, S, F, verify_pages=0):
 @pytest.mark.parametrize("kw", [dict(), dict(layout="layer", policy=1), dict(num_blocks=160, host_slots=48),
                                 dict(num_blocks=128, host_slots=256, use_hint=True, max_admit=3),
                                 dict(num_blocks=160, host_slots=32, policy=2, evict_policy="lru"),
-                                dict(num_blocks=160, host_slots=32, policy=2, evict_policy="infercept")])
+                                dict(num_blocks=160, host_slots=32, policy=2, evict_policy="infercept"),
+                                dict(num_blocks=160, host_slots=48, token_budget=512, max_admit=4, offload="auto")])
 def test_gpu_tiny_replay_is_bit_exact(kw):
     tr = gen.tiny_trace(0)
     cfg = tiny_cfg(**kw)

@@ -33,6 +33,7 @@ namespace {
 #define CWE_ITEMS 2  // measured: 2 -> 80 us, 3 -> 82, 4 -> 83, 6 -> 86 (configs[2], whole kernel)
 #define CWE_TILE (CWE_THREADS * CWE_ITEMS)
 #define CWE_SMEM_SESS 4096                       // sessions whose tau fits the per-CTA shared-memory table
+#define CWE_RANK_SESS 512                        // up to here level 0 resolves tau COMPLETELY (digit = rank of the session's tau)
 #define CWE_SMEM_SORT (CWE_SORT_RUN * 24)        // two (score,id) buffers of the CTA sort (alias the histogram)
 #define CWE_SMEM_BYTES (CWE_SMEM_SORT + CWE_SMEM_SESS * 4)
 
@@ -174,6 +175,18 @@ __device__ __forceinline__ void make_plan(DigitPlan* pl, u64 vary_hi, u32 vary_l
     if (lane == 0) {
         pl->nbits = n;
         pl->nruns = runs;
+    }
+}
+
+// the key bits a plan reads, as masks over (score : id)
+__device__ __forceinline__ void plan_bits(const DigitPlan& pl, u64& hi, u32& lo) {
+    hi = 0;
+    lo = 0;
+    for (u32 r = 0; r < pl.nruns; ++r) {
+        const u64 m = (u64)pl.mask[r] << pl.shift[r];
+        if (pl.word[r] == 2) hi |= m << 32;
+        else if (pl.word[r] == 1) hi |= m;
+        else lo |= (u32)m;
     }
 }
 
@@ -405,7 +418,8 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     __shared__ u32 s_mlo[4 * CWE_WARPS];
     __shared__ u64 s_acc_hi, s_acc2_hi;
     __shared__ u32 s_acc_lo, s_acc2_lo, s_cnt[2];
-    __shared__ DigitPlan s_plan;
+    __shared__ DigitPlan s_plan, s_plan2;
+    __shared__ unsigned short s_rank[CWE_RANK_SESS];  // level-0 digit of a session in rank mode
     const u32 tid = threadIdx.x, G = gridDim.x;
     cw_evict_state* st = a.st;
     const bool tau_smem = a.S <= CWE_SMEM_SESS;
@@ -479,43 +493,91 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
         __syncthreads();
     }
 
+    // Rank mode (S <= 512): the level-0 digit of a block is the number of sessions whose tau is LARGER than its
+    // session's (one prediction per session) — monotone in the score's tau field and injective on it, so
+    // level 0 resolves all 24 tau bits at once, whatever their bit patterns, and the threshold set holds ONE tau value.
+    const bool rank_mode = tau_smem && a.S <= CWE_RANK_SESS;
+    if (rank_mode) {
+        for (u32 sidx = tid >> 5; sidx < a.S; sidx += CWE_WARPS) {  // one warp per session, the lanes share the scan
+            const u32 mine = s_tau[sidx];
+            u32 larger = 0;
+            for (u32 j = tid & 31; j < a.S; j += 32) larger += s_tau[j] > mine ? 1u : 0u;
+            larger = __reduce_add_sync(0xffffffffu, larger);
+            if ((tid & 31) == 0) s_rank[sidx] = (unsigned short)larger;
+        }
+        __syncthreads();
+    }
     stamp(st, n_stamp);  // end of phase A
-    // ---------------------------------------------------------------- B: score + compact + level-0 histogram
+    // ---------------------------------------------------------------- B: score + level-0 histogram
+    // Nothing is written here: the candidates are NOT materialised (835 k of the 1 M blocks of configs[2] are evictable:
+    // 10 MB out and back, and three block-wide barriers per tile for the compaction).  The level-0 filter re-reads the
+    // metadata instead (16 MB, L2-resident by then) and recomputes the scores.  What the pass does collect: the level-0
+    // histogram, the number of evictable blocks, and the bits that vary over ALL evictable keys (for the level-1 plan).
     for (u32 i = tid; i < CWE_BINS; i += CWE_THREADS) s_hist[i] = 0;
     __syncthreads();
+    auto block_score = [&](u32 k) -> u64 {  // rf/se/la/dp[k] hold the metadata of one evictable block
+        const u32 tau = se[k] < a.S ? (tau_smem ? s_tau[se[k]] : __ldcg(a.tau_q + se[k])) : CW_TAU_MAX;
+        const u32 age = min(a.tick_now >= la[k] ? a.tick_now - la[k] : 0u, 0xFFFFFu);
+        const u32 dpc = min(dp[k], 0xFFFFFu);
+        return ((u64)(CW_TAU_MAX - tau) << 40) | ((u64)(0xFFFFFu - age) << 20) | (u64)(0xFFFFFu - dpc);
+    };
+    auto digit0 = [&](u32 k, u64 sc, u32 b) -> u32 {  // level-0 digit of the block whose metadata sits in slot k
+        if (rank_mode) return se[k] < a.S ? (u32)s_rank[se[k]] : 0u;  // unknown session: tau = TAU_MAX, nobody is larger
+        return plan_digit(s_plan, sc, b);
+    };
+    auto evictable = [&](u32 k) -> bool {
+        return (rf[k] & CW_REF_VALID) && !(rf[k] & CW_REF_PINNED) && (rf[k] & 0x3FFFFFFFu) == 0;
+    };
     {
-        const DigitPlan& pl = s_plan;
+        u64 a_or_hi = 0, a_nand_hi = 0;
+        u32 a_or_lo = 0, a_nand_lo = 0, my_cnt = 0;
         for (u32 tile = blockIdx.x; (u64)tile * CWE_TILE < a.M; tile += G) {
-            bool f0[CWE_ITEMS], f1[CWE_ITEMS];
-            u32 p0[CWE_ITEMS], p1[CWE_ITEMS];
-            u64 sc[CWE_ITEMS];
-            if (tile != blockIdx.x) load_tile(tile);
+            // the current tile moves to private registers and the NEXT tile's metadata is requested at once: its
+            // latency hides behind this tile's scoring and histogram
+            bool ev_c[CWE_ITEMS];
+            u64 sc_c[CWE_ITEMS];
+#pragma unroll
+            for (int k = 0; k < CWE_ITEMS; ++k) {
+                ev_c[k] = evictable(k);
+                sc_c[k] = ev_c[k] ? block_score(k) : 0ull;
+            }
+            u32 dg_c[CWE_ITEMS];
+#pragma unroll
+            for (int k = 0; k < CWE_ITEMS; ++k)
+                dg_c[k] = ev_c[k] ? digit0(k, sc_c[k], tile * CWE_TILE + k * CWE_THREADS + tid) : 0u;
+            load_tile(tile + G);  // out-of-range tiles load nothing
 #pragma unroll
             for (int k = 0; k < CWE_ITEMS; ++k) {
                 const u32 b = tile * CWE_TILE + k * CWE_THREADS + tid;
-                f0[k] = false;
-                f1[k] = false;
-                sc[k] = 0;
-                if ((rf[k] & CW_REF_VALID) && !(rf[k] & CW_REF_PINNED) && (rf[k] & 0x3FFFFFFFu) == 0) {
-                    const u32 tau = se[k] < a.S ? (tau_smem ? s_tau[se[k]] : __ldcg(a.tau_q + se[k])) : CW_TAU_MAX;
-                    const u32 age = min(a.tick_now >= la[k] ? a.tick_now - la[k] : 0u, 0xFFFFFu);
-                    const u32 dpc = min(dp[k], 0xFFFFFu);
-                    sc[k] = ((u64)(CW_TAU_MAX - tau) << 40) | ((u64)(0xFFFFFu - age) << 20) | (u64)(0xFFFFFu - dpc);
-                    f0[k] = true;
+                const bool ev = ev_c[k];
+                const u64 sc = sc_c[k];
+                hist_add(s_hist, ev, dg_c[k]);
+                if (ev) {
+                    a_or_hi |= sc;
+                    a_nand_hi |= ~sc;
+                    a_or_lo |= b;
+                    a_nand_lo |= ~b;
+                    ++my_cnt;
                 }
-                hist_add(s_hist, f0[k], f0[k] ? plan_digit(pl, sc[k], b) : 0u);
             }
-            tile_append(f0, f1, p0, p1, &st->n_cand[0], &st->n_cand[0], s_w0, s_w1, s_base);
-#pragma unroll
-            for (int k = 0; k < CWE_ITEMS; ++k)
-                if (f0[k]) {
-                    a.cand_score[0][p0[k]] = sc[k];
-                    a.cand_id[0][p0[k]] = tile * CWE_TILE + k * CWE_THREADS + tid;
-                }
+        }
+        stamp(st, n_stamp);  // CTA 0 done with its tiles
+        flush_hist(s_hist, a.hist);
+        {
+            const u64 h2[2] = {a_or_hi, a_nand_hi};
+            const u32 l2[2] = {a_or_lo, a_nand_lo};
+            u64* const gh[2] = {&st->all_or_hi, &st->all_nand_hi};
+            u32* const gl[2] = {&st->all_or_lo, &st->all_nand_lo};
+            block_or_n<2>(h2, l2, gh, gl, s_mhi, s_mlo);
+        }
+        my_cnt = __reduce_add_sync(0xffffffffu, my_cnt);
+        if ((tid & 31) == 0) s_w0[tid >> 5] = my_cnt;
+        __syncthreads();
+        if (tid < 32) {
+            const u32 c = __reduce_add_sync(0xffffffffu, s_w0[tid]);
+            if (tid == 0 && c) atomicAdd(&st->n_cand[0], c);
         }
     }
-    stamp(st, n_stamp);  // CTA 0 done with its tiles
-    flush_hist(s_hist, a.hist);
     grid_barrier(st, G, bar_gen);
     stamp(st, n_stamp);
 
@@ -531,8 +593,145 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     }
     u32 remaining = want;
     u32 n_cur = n_evictable;
-    if (want > 0) {
-        for (int p = 0;; ++p) {
+    int p_first = 0;
+    if (want > 0 && n_evictable <= CWE_LOCAL) {
+        // small candidate set: materialise it (one more pass over the metadata) and let one CTA finish it below
+        for (u32 tile = blockIdx.x; (u64)tile * CWE_TILE < a.M; tile += G) {
+            bool f0[CWE_ITEMS], f1[CWE_ITEMS];
+            u32 p0[CWE_ITEMS], p1[CWE_ITEMS];
+            u64 sc[CWE_ITEMS];
+            load_tile(tile);
+#pragma unroll
+            for (int k = 0; k < CWE_ITEMS; ++k) {
+                f0[k] = evictable(k);
+                f1[k] = false;
+                sc[k] = f0[k] ? block_score(k) : 0ull;
+            }
+            tile_append(f0, f1, p0, p1, &st->cursor0, &st->cursor0, s_w0, s_w1, s_base);
+#pragma unroll
+            for (int k = 0; k < CWE_ITEMS; ++k)
+                if (f0[k]) {
+                    a.cand_score[0][p0[k]] = sc[k];
+                    a.cand_id[0][p0[k]] = tile * CWE_TILE + k * CWE_THREADS + tid;
+                }
+        }
+        grid_barrier(st, G, bar_gen);
+        stamp(st, n_stamp);
+    } else if (want > 0) {
+        // ---- level 0, straight from the metadata, FUSED with the level-1 histogram.  The level-1 digit is taken from
+        // the bits that vary over all evictable keys and that level 0 did not use (a static plan: it is known before
+        // the threshold set exists, so the set's histogram can be built while the set is written: one grid barrier
+        // and one pass less than "filter, reduce the masks, barrier, histogram, barrier").
+        find_threshold<true>(a.hist, remaining, s_scan, s_thr);
+        const u32 thr = s_thr[0], before = s_thr[1], inside = s_thr[2];
+        const u32 need_here = remaining - before;
+        const bool take_all = need_here == inside;
+        const bool next = !take_all && inside > CWE_LOCAL;  // a level-1 pass over the grid will follow
+        if (tid < 32) {
+            u64 used_hi;
+            u32 used_lo;
+            plan_bits(s_plan, used_hi, used_lo);
+            if (rank_mode) {  // level 0 consumed the whole tau field
+                used_hi = 0xFFFFFF0000000000ull;
+                used_lo = 0;
+            }
+            const u64 vh = __ldcg(reinterpret_cast<const unsigned long long*>(&st->all_or_hi)) &
+                           __ldcg(reinterpret_cast<const unsigned long long*>(&st->all_nand_hi)) & ~used_hi;
+            const u32 vl = __ldcg(&st->all_or_lo) & __ldcg(&st->all_nand_lo) & ~used_lo;
+            make_plan(&s_plan2, vh, vl, 96);
+        }
+        for (u32 i = tid; i < CWE_BINS; i += CWE_THREADS) s_hist[i] = 0;
+        __syncthreads();
+        stamp(st, n_stamp);  // threshold found
+        {
+            const DigitPlan& pn = s_plan2;
+            u64 m_or_hi = 0, m_nand_hi = 0, v_or_hi = 0, v_nand_hi = 0;  // next candidate set / victims
+            u32 m_or_lo = 0, m_nand_lo = 0, v_or_lo = 0, v_nand_lo = 0;
+            load_tile(blockIdx.x);
+            for (u32 tile = blockIdx.x; (u64)tile * CWE_TILE < a.M; tile += G) {
+                bool f0[CWE_ITEMS], f1[CWE_ITEMS];
+                u32 p0[CWE_ITEMS], p1[CWE_ITEMS];
+                u64 sc[CWE_ITEMS];
+                u32 dg0[CWE_ITEMS];
+                bool ev[CWE_ITEMS];
+#pragma unroll
+                for (int k = 0; k < CWE_ITEMS; ++k) {  // consume the tile's registers, then request the next tile
+                    ev[k] = evictable(k);
+                    sc[k] = ev[k] ? block_score(k) : 0ull;
+                    dg0[k] = ev[k] ? digit0(k, sc[k], tile * CWE_TILE + k * CWE_THREADS + tid) : 0u;
+                }
+                load_tile(tile + G);
+#pragma unroll
+                for (int k = 0; k < CWE_ITEMS; ++k) {
+                    const u32 b = tile * CWE_TILE + k * CWE_THREADS + tid;
+                    f0[k] = f1[k] = false;
+                    if (ev[k]) {
+                        const u32 dg = dg0[k];
+                        if (dg < thr || (take_all && dg == thr)) {
+                            f0[k] = true;
+                            v_or_hi |= sc[k];
+                            v_nand_hi |= ~sc[k];
+                            v_or_lo |= b;
+                            v_nand_lo |= ~b;
+                        } else if (dg == thr) {
+                            f1[k] = true;
+                            m_or_hi |= sc[k];
+                            m_nand_hi |= ~sc[k];
+                            m_or_lo |= b;
+                            m_nand_lo |= ~b;
+                        }
+                    }
+                    if (next) hist_add(s_hist, f1[k], f1[k] ? plan_digit(pn, sc[k], b) : 0u);
+                }
+                tile_append(f0, f1, p0, p1, &st->n_out, &st->n_cand[1], s_w0, s_w1, s_base);
+#pragma unroll
+                for (int k = 0; k < CWE_ITEMS; ++k) {
+                    const u32 b = tile * CWE_TILE + k * CWE_THREADS + tid;
+                    if (f0[k]) {
+                        a.out_score[p0[k]] = sc[k];
+                        a.out_id[p0[k]] = b;
+                    } else if (f1[k]) {
+                        a.cand_score[1][p1[k]] = sc[k];
+                        a.cand_id[1][p1[k]] = b;
+                    }
+                }
+            }
+            stamp(st, n_stamp);  // CTA 0 done with its filter tiles
+            if (next) flush_hist(s_hist, a.hist + CWE_BINS);
+            const u64 h4[4] = {v_or_hi, v_nand_hi, next ? m_or_hi : 0ull, next ? m_nand_hi : 0ull};
+            const u32 l4[4] = {v_or_lo, v_nand_lo, next ? m_or_lo : 0u, next ? m_nand_lo : 0u};
+            u64* const gh[4] = {&st->vic_or_hi, &st->vic_nand_hi, &st->or_hi[1], &st->nand_hi[1]};
+            u32* const gl[4] = {&st->vic_or_lo, &st->vic_nand_lo, &st->or_lo[1], &st->nand_lo[1]};
+            block_or_n<4>(h4, l4, gh, gl, s_mhi, s_mlo);
+        }
+        grid_barrier(st, G, bar_gen);
+        stamp(st, n_stamp);
+        if (take_all) {
+            remaining = 0;
+        } else {
+            remaining = need_here;
+            n_cur = inside;
+            p_first = 1;
+            if (tid < 32) {  // level 1 reads its digits with the static plan
+                DigitPlan* d = &s_plan;
+                const DigitPlan* c = &s_plan2;
+                const u32 lane = tid;
+                if (lane < CWE_BUCKET_BITS) {
+                    d->word[lane] = c->word[lane];
+                    d->shift[lane] = c->shift[lane];
+                    d->mask[lane] = c->mask[lane];
+                    d->dst[lane] = c->dst[lane];
+                }
+                if (lane == 0) {
+                    d->nbits = c->nbits;
+                    d->nruns = c->nruns;
+                }
+            }
+            __syncthreads();
+        }
+    }
+    if (want > 0 && remaining > 0) {
+        for (int p = p_first;; ++p) {
             const u64* cs = a.cand_score[p & 1];
             const u32* ci = a.cand_id[p & 1];
             if (n_cur <= CWE_LOCAL || p >= CWE_PASSES) {

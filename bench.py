@@ -615,6 +615,16 @@ def run_cuda(args):
     del st
     torch.cuda.empty_cache()
 
+    if world > 1 and not args.quick and not args.no_swap_sweep:
+        # tensor-parallel stage 4 (TP=2): every rank swaps its own KV-head slice over its own PCIe link
+        from harness import tp as htp
+        try:
+            tp_rows = htp.tp_swap_sweep(torch, cw, gen, hdist, stream, rank, world)
+        except Exception as e:
+            tp_rows = {"error": repr(e)[:300]}
+        if rank == 0:
+            extra["swap_sweep_tp"] = tp_rows
+
     if rank == 0:
         pcie = pcie_peak(torch, stream)
         extra["pcie_peak"] = dict(pcie, gen5_x16_raw_gbs=PCIE_GEN5_X16_GBS)

@@ -131,3 +131,37 @@ def test_bench_gpus_2_launches_two_ranks():
     line = [l for l in out.stdout.splitlines() if l.startswith("{")][-1]
     d = json.loads(line)
     assert d["n_gpus"] == 2 and d["units"] == 3000.0 and d["max_ms"] == 20.0
+
+
+def test_tp_head_slices_partition_the_page_and_reassemble_through_the_oracle():
+    """SURVEY.md 8f NEXT-4 (TP=2): stage 4 shards by KV head with no exchange.  Host logic only (the
+    GPU halves are in test_gpu_evict_swap.py): the slices partition every chunk, and the ranks' oracle swap-outs of
+    their shards, re-interleaved, are the oracle's swap-out of the unsharded pool, for both pool layouts."""
+    import numpy as np
+    import oracle
+    from harness import gen, tp as htp
+    M, n_chunks, cb, n = 24, 4, 256, 9
+    g = gen.rng(91, 0)
+    full = g.integers(0, 256, size=(n_chunks, M, cb), dtype=np.uint8)
+    vic = g.permutation(M)[:n].astype(np.uint32)
+    exp = oracle.swap_out(full.reshape(-1).copy(), n_chunks, cb, M * cb, cb, vic, np.zeros(n * n_chunks * cb, np.uint8))
+    for tp in (1, 2, 4, 8):
+        cover = np.zeros(cb, np.int32)
+        pages = []
+        for r in range(tp):
+            off, sb = htp.head_slice(cb, tp, r)
+            cover[off:off + sb] += 1
+            for layout in ("layer", "block"):
+                shard = htp.shard_pool(full, tp, r, layout)
+                cs, bs = (M * sb, sb) if layout == "layer" else (sb, n_chunks * sb)
+                out = oracle.swap_out(shard, n_chunks, sb, cs, bs, vic, np.zeros(n * n_chunks * sb, np.uint8))
+                if layout == "layer":
+                    pages.append(out)
+                else:
+                    assert np.array_equal(out, pages[-1])          # the layout does not change the staged page
+        assert (cover == 1).all()
+        assert np.array_equal(htp.interleave_pages(pages, n, n_chunks).reshape(-1), exp)
+    with pytest.raises(ValueError):
+        htp.head_slice(cb, 3, 0)
+    with pytest.raises(ValueError):
+        htp.head_slice(cb, 2, 2)

@@ -322,21 +322,19 @@ def test_tp_sharded_swap_equals_the_unsharded_page(layout, tp):
     vic = g.permutation(M)[:n].astype(np.uint32)
     exp = oracle.swap_out(full.reshape(-1).copy(), n_chunks, cb, full_cfg["chunk_stride"], full_cfg["block_stride"], vic,
                           np.zeros(n * n_chunks * cb, np.uint8)).reshape(n, n_chunks, cb)
+    from harness import tp as htp
     sb = cb // tp
     pages, ctxs = [], []
     for t in range(tp):
-        shard = full[:, :, t * sb:(t + 1) * sb]                               # rank t's head slice
-        if layout == "layer_major":
-            pool_np = np.ascontiguousarray(shard).reshape(-1)
-        else:
-            pool_np = np.ascontiguousarray(shard.transpose(1, 0, 2)).reshape(-1)
+        assert htp.head_slice(cb, tp, t) == (t * sb, sb)
+        pool_np = htp.shard_pool(full, tp, t, "layer" if layout == "layer_major" else "block")  # rank t's head slice
         ctx, pool = _swap_ctx(layout, M, n_chunks, sb, 4, pool_np)
         h = torch.zeros(n * n_chunks * sb, dtype=torch.uint8).pin_memory()
         ctx.swap_out(dev(vic), None, n, None, h)
         assert ctx.sync(check=False) == 0
         pages.append(h.numpy().reshape(n, n_chunks, sb).copy())
         ctxs.append((ctx, pool, pool_np, h))
-    assert (np.concatenate(pages, axis=2) == exp).all()
+    assert (htp.interleave_pages(pages, n, n_chunks) == exp).all()
     for ctx, pool, pool_np, h in ctxs:                                        # restore into wiped pools
         pool.zero_()
         ctx.swap_in(None, h, dev(vic), n)

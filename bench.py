@@ -57,7 +57,8 @@ def ncu_traffic():
             if len(r) <= max(ki, ri, wi):
                 continue
             for stage, kern in STAGE_KERNEL.items():
-                name = r[ki].replace("(bool)1", "true").replace("(bool)0", "false")
+                name = (r[ki].replace("(bool)1", "true").replace("(bool)0", "false")
+                        .replace("kernel<1>", "kernel<true>").replace("kernel<0>", "kernel<false>"))
                 if kern in name:
                     out[stage] = int(float(r[ri]) * scale.get(units[ri], 1.0) + float(r[wi]) * scale.get(units[wi], 1.0))
         return out

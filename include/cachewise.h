@@ -90,6 +90,10 @@ const char* cw_last_error(cw_ctx* ctx);
  * grid-wide phases; h_out32[31] = how many are valid.  Debug builds also reject duplicate block ids in
  * cw_swap_out / cw_gather_pages (CW_E_INVAL at cw_sync; SURVEY.md 8c stage 4). */
 int32_t cw_debug_evict_times(cw_ctx* ctx, uint64_t* h_out32);
+/* cw_debug_stamp queues a one-thread kernel on stream_main that stores %globaltimer in slot i (< 32); cw_debug_stamps
+ * waits and copies the 32 slots: with cw_debug_evict_times (same clock) this gives the timeline of a step's branches. */
+int32_t cw_debug_stamp(cw_ctx* ctx, uint32_t i);
+int32_t cw_debug_stamps(cw_ctx* ctx, uint64_t* h_out32);
 #endif
 /* Number of kernels this ctx has launched so far (bench.py's gpu_launches). */
 uint64_t cw_launch_count(const cw_ctx* ctx);

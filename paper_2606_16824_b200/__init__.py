@@ -28,7 +28,7 @@ EXPORTS = ["cw_create", "cw_destroy", "cw_sync", "cw_join_copy", "cw_last_error"
            "cw_predict_tau", "cw_swap_out", "cw_swap_in", "cw_gather_pages", "cw_scatter_pages", "cw_table_insert",
            "cw_table_erase", "cw_table_retag", "cw_table_lookup", "cw_table_compact", "cw_table_stats",
            "cw_blocks_update"]
-DEBUG_EXPORTS = ["cw_debug_evict_times"]  # libcachewise_debug.so only
+DEBUG_EXPORTS = ["cw_debug_evict_times", "cw_debug_stamp", "cw_debug_stamps"]  # libcachewise_debug.so only
 
 
 class CwConfig(C.Structure):
@@ -65,6 +65,10 @@ def lib():
         if DEBUG:
             L.cw_debug_evict_times.argtypes = [P, P]
             L.cw_debug_evict_times.restype = I32
+            L.cw_debug_stamp.argtypes = [P, U32]
+            L.cw_debug_stamp.restype = I32
+            L.cw_debug_stamps.argtypes = [P, P]
+            L.cw_debug_stamps.restype = I32
         L.cw_last_error.argtypes = [P]
         L.cw_last_error.restype = C.c_char_p
         L.cw_launch_count.argtypes = [P]
@@ -160,6 +164,22 @@ class Context:
         self._ck(lib().cw_debug_evict_times(self._h, buf), "cw_debug_evict_times")
         n = min(int(buf[31]), 31)
         return [int(buf[i]) - int(buf[0]) for i in range(n)]
+
+    def debug_timeline(self, fn_list):
+        """Debug build: runs the callables in order with a %globaltimer stamp on stream_main before the first and after
+        each; returns (main-stream stamps in ns, absolute stamps of the last evict kernel in ns)."""
+        if not DEBUG:
+            raise CwError(CW_E_STATE, "debug_timeline", "needs the debug library (CACHEWISE_DEBUG=1)")
+        L = lib()
+        self._ck(L.cw_debug_stamp(self._h, 0), "cw_debug_stamp")
+        for i, f in enumerate(fn_list):
+            f()
+            self._ck(L.cw_debug_stamp(self._h, i + 1), "cw_debug_stamp")
+        buf, ev = (C.c_uint64 * 32)(), (C.c_uint64 * 32)()
+        self._ck(L.cw_debug_stamps(self._h, buf), "cw_debug_stamps")
+        self._ck(L.cw_debug_evict_times(self._h, ev), "cw_debug_evict_times")
+        n = min(int(ev[31]), 31)
+        return [int(buf[i]) for i in range(len(fn_list) + 1)], [int(ev[i]) for i in range(n)]
 
     @property
     def launches(self):

@@ -41,6 +41,7 @@ void free_all(cw_ctx* c) {
     if (c->s_side) cudaStreamDestroy(c->s_side);
     cudaFree(c->spec_n);
     cudaFree(c->dup_bits);
+    cudaFree(c->dbg_stamps);
     cudaFree(c->d_status);
     if (c->h_status) cudaFreeHost(c->h_status);
     cudaFree(c->hash_unit_off);
@@ -163,6 +164,7 @@ int32_t cw_create(const cw_config* cfg, cw_ctx** out) {
     CW_CUDA(c, cudaEventCreateWithFlags(&c->ev_spec, cudaEventDisableTiming));
 #ifdef CW_DEBUG
     CW_CUDA(c, dalloc_zero(&c->dup_bits, ((size_t)cfg->num_blocks + 31) / 32, s));
+    CW_CUDA(c, dalloc_zero(&c->dbg_stamps, 32, s));
 #endif
     // stage 4
     if (cfg->staging_bytes) {
@@ -215,10 +217,30 @@ int32_t cw_join_copy(cw_ctx* ctx) {
 }
 
 #ifdef CW_DEBUG
+__global__ void debug_stamp_kernel(u64* slot) {
+    u64 t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    *slot = t;
+}
+int32_t cw_debug_stamp(cw_ctx* ctx, uint32_t i) {
+    if (!ctx) return CW_E_STATE;
+    if (i >= 32) return CW_E_INVAL;
+    debug_stamp_kernel<<<1, 1, 0, ctx->s_main>>>(ctx->dbg_stamps + i);
+    return CW_OK;
+}
+int32_t cw_debug_stamps(cw_ctx* ctx, uint64_t* h_out32) {
+    if (!ctx) return CW_E_STATE;
+    if (!h_out32) return CW_E_INVAL;
+    CW_CUDA(ctx, cudaStreamSynchronize(ctx->s_main));
+    CW_CUDA(ctx, cudaStreamSynchronize(ctx->s_side));
+    CW_CUDA(ctx, cudaMemcpy(h_out32, ctx->dbg_stamps, 32 * sizeof(u64), cudaMemcpyDeviceToHost));
+    return CW_OK;
+}
 int32_t cw_debug_evict_times(cw_ctx* ctx, uint64_t* h_out32) {
     if (!ctx) return CW_E_STATE;
     if (!h_out32) return CW_E_INVAL;
     CW_CUDA(ctx, cudaStreamSynchronize(ctx->s_main));
+    CW_CUDA(ctx, cudaStreamSynchronize(ctx->s_side));
     CW_CUDA(ctx, cudaMemcpy(h_out32, reinterpret_cast<uint8_t*>(ctx->ev) + offsetof(cw_evict_state, stamps),
                             CWE_STAMPS * sizeof(u64), cudaMemcpyDeviceToHost));
     return CW_OK;

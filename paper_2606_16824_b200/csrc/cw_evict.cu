@@ -32,6 +32,9 @@ namespace {
 #define CWE_WARPS (CWE_THREADS / 32)
 #define CWE_ITEMS 2  // measured: 2 -> 80 us, 3 -> 82, 4 -> 83, 6 -> 86 (configs[2], whole kernel)
 #define CWE_TILE (CWE_THREADS * CWE_ITEMS)
+#define CWE_MI 4     // blocks per thread and tile in the passes over the metadata: four CONSECUTIVE blocks, one 128-bit
+                     // load per array (64 bytes in flight per thread: a reduced grid is bound by bytes in flight per SM)
+#define CWE_MTILE (CWE_THREADS * CWE_MI)
 #define CWE_SMEM_SESS 4096                       // sessions whose tau fits the per-CTA shared-memory table
 #define CWE_RANK_SESS 512                        // up to here level 0 resolves tau COMPLETELY (digit = rank of the session's tau)
 #define CWE_SMEM_SORT (CWE_SORT_RUN * 24)        // two (score,id) buffers of the CTA sort (alias the histogram)
@@ -265,14 +268,15 @@ __device__ __forceinline__ void hist_add(u32* s_hist, bool valid, u32 digit) {
 }
 
 // Block-cooperative compaction of one tile: flags f0 (-> list 0) and f1 (-> list 1) per item.
-__device__ __forceinline__ void tile_append(const bool (&f0)[CWE_ITEMS], const bool (&f1)[CWE_ITEMS],
-                                            u32 (&pos0)[CWE_ITEMS], u32 (&pos1)[CWE_ITEMS], u32* ctr0, u32* ctr1,
+template <int NI>
+__device__ __forceinline__ void tile_append(const bool (&f0)[NI], const bool (&f1)[NI],
+                                            u32 (&pos0)[NI], u32 (&pos1)[NI], u32* ctr0, u32* ctr1,
                                             u32* s_w0, u32* s_w1, u32* s_base) {
     const u32 lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     u32 c0 = 0, c1 = 0;
-    u32 r0[CWE_ITEMS], r1[CWE_ITEMS];
+    u32 r0[NI], r1[NI];
 #pragma unroll
-    for (int k = 0; k < CWE_ITEMS; ++k) {
+    for (int k = 0; k < NI; ++k) {
         const u32 b0 = __ballot_sync(0xffffffffu, f0[k]);
         const u32 b1 = __ballot_sync(0xffffffffu, f1[k]);
         r0[k] = c0 + __popc(b0 & ((1u << lane) - 1));
@@ -306,7 +310,7 @@ __device__ __forceinline__ void tile_append(const bool (&f0)[CWE_ITEMS], const b
     __syncthreads();
     const u32 o0 = s_base[0] + s_w0[warp], o1 = s_base[1] + s_w1[warp];
 #pragma unroll
-    for (int k = 0; k < CWE_ITEMS; ++k) {
+    for (int k = 0; k < NI; ++k) {
         pos0[k] = o0 + r0[k];
         pos1[k] = o1 + r1[k];
     }
@@ -428,16 +432,28 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     stamp(st, n_stamp);
 
     // the metadata of this CTA's first tile is requested before phase A: its DRAM latency hides behind the tau pass
-    u32 rf[CWE_ITEMS], se[CWE_ITEMS], la[CWE_ITEMS], dp[CWE_ITEMS];
+    u32 rf[CWE_MI], se[CWE_MI], la[CWE_MI], dp[CWE_MI];
     auto load_tile = [&](u32 tile) {
+        const u64 b0 = (u64)tile * CWE_MTILE + (u64)tid * CWE_MI;  // four consecutive blocks: 16-byte aligned in every array
+        if (b0 + CWE_MI <= a.M) {
+            const uint4 r4 = *reinterpret_cast<const uint4*>(a.m_ref + b0);
+            const uint4 s4 = *reinterpret_cast<const uint4*>(a.m_session + b0);
+            const uint4 l4 = *reinterpret_cast<const uint4*>(a.m_last + b0);
+            const uint4 d4 = *reinterpret_cast<const uint4*>(a.m_depth + b0);
+            rf[0] = r4.x; rf[1] = r4.y; rf[2] = r4.z; rf[3] = r4.w;
+            se[0] = s4.x; se[1] = s4.y; se[2] = s4.z; se[3] = s4.w;
+            la[0] = l4.x; la[1] = l4.y; la[2] = l4.z; la[3] = l4.w;
+            dp[0] = d4.x; dp[1] = d4.y; dp[2] = d4.z; dp[3] = d4.w;
+        } else {
 #pragma unroll
-        for (int k = 0; k < CWE_ITEMS; ++k) {
-            const u32 b = tile * CWE_TILE + k * CWE_THREADS + tid;
-            const bool in = (u64)tile * CWE_TILE < a.M && b < a.M;
-            rf[k] = in ? a.m_ref[b] : 0u;
-            se[k] = in ? a.m_session[b] : 0u;
-            la[k] = in ? a.m_last[b] : 0u;
-            dp[k] = in ? a.m_depth[b] : 0u;
+            for (int k = 0; k < CWE_MI; ++k) {  // ragged end of the pool (or a tile past it: nothing is loaded)
+                const u64 b = b0 + k;
+                const bool in = b < a.M;
+                rf[k] = in ? a.m_ref[b] : 0u;
+                se[k] = in ? a.m_session[b] : 0u;
+                la[k] = in ? a.m_last[b] : 0u;
+                dp[k] = in ? a.m_depth[b] : 0u;
+            }
         }
     };
     load_tile(blockIdx.x);
@@ -531,34 +547,22 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     {
         u64 a_or_hi = 0, a_nand_hi = 0;
         u32 a_or_lo = 0, a_nand_lo = 0, my_cnt = 0;
-        for (u32 tile = blockIdx.x; (u64)tile * CWE_TILE < a.M; tile += G) {
-            // the current tile moves to private registers and the NEXT tile's metadata is requested at once: its
-            // latency hides behind this tile's scoring and histogram
-            bool ev_c[CWE_ITEMS];
-            u64 sc_c[CWE_ITEMS];
+        for (u32 tile = blockIdx.x; (u64)tile * CWE_MTILE < a.M; tile += G) {
+            if (tile != blockIdx.x) load_tile(tile);
 #pragma unroll
-            for (int k = 0; k < CWE_ITEMS; ++k) {
-                ev_c[k] = evictable(k);
-                sc_c[k] = ev_c[k] ? block_score(k) : 0ull;
-            }
-            u32 dg_c[CWE_ITEMS];
-#pragma unroll
-            for (int k = 0; k < CWE_ITEMS; ++k)
-                dg_c[k] = ev_c[k] ? digit0(k, sc_c[k], tile * CWE_TILE + k * CWE_THREADS + tid) : 0u;
-            load_tile(tile + G);  // out-of-range tiles load nothing
-#pragma unroll
-            for (int k = 0; k < CWE_ITEMS; ++k) {
-                const u32 b = tile * CWE_TILE + k * CWE_THREADS + tid;
-                const bool ev = ev_c[k];
-                const u64 sc = sc_c[k];
-                hist_add(s_hist, ev, dg_c[k]);
+            for (int k = 0; k < CWE_MI; ++k) {
+                const u32 b = tile * CWE_MTILE + tid * CWE_MI + k;
+                const bool ev = evictable(k);
+                u64 sc = 0;
                 if (ev) {
+                    sc = block_score(k);
                     a_or_hi |= sc;
                     a_nand_hi |= ~sc;
                     a_or_lo |= b;
                     a_nand_lo |= ~b;
                     ++my_cnt;
                 }
+                hist_add(s_hist, ev, ev ? digit0(k, sc, b) : 0u);
             }
         }
         stamp(st, n_stamp);  // CTA 0 done with its tiles
@@ -596,23 +600,23 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     int p_first = 0;
     if (want > 0 && n_evictable <= CWE_LOCAL) {
         // small candidate set: materialise it (one more pass over the metadata) and let one CTA finish it below
-        for (u32 tile = blockIdx.x; (u64)tile * CWE_TILE < a.M; tile += G) {
-            bool f0[CWE_ITEMS], f1[CWE_ITEMS];
-            u32 p0[CWE_ITEMS], p1[CWE_ITEMS];
-            u64 sc[CWE_ITEMS];
+        for (u32 tile = blockIdx.x; (u64)tile * CWE_MTILE < a.M; tile += G) {
+            bool f0[CWE_MI], f1[CWE_MI];
+            u32 p0[CWE_MI], p1[CWE_MI];
+            u64 sc[CWE_MI];
             load_tile(tile);
 #pragma unroll
-            for (int k = 0; k < CWE_ITEMS; ++k) {
+            for (int k = 0; k < CWE_MI; ++k) {
                 f0[k] = evictable(k);
                 f1[k] = false;
                 sc[k] = f0[k] ? block_score(k) : 0ull;
             }
             tile_append(f0, f1, p0, p1, &st->cursor0, &st->cursor0, s_w0, s_w1, s_base);
 #pragma unroll
-            for (int k = 0; k < CWE_ITEMS; ++k)
+            for (int k = 0; k < CWE_MI; ++k)
                 if (f0[k]) {
                     a.cand_score[0][p0[k]] = sc[k];
-                    a.cand_id[0][p0[k]] = tile * CWE_TILE + k * CWE_THREADS + tid;
+                    a.cand_id[0][p0[k]] = tile * CWE_MTILE + tid * CWE_MI + k;
                 }
         }
         grid_barrier(st, G, bar_gen);
@@ -647,26 +651,19 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
             const DigitPlan& pn = s_plan2;
             u64 m_or_hi = 0, m_nand_hi = 0, v_or_hi = 0, v_nand_hi = 0;  // next candidate set / victims
             u32 m_or_lo = 0, m_nand_lo = 0, v_or_lo = 0, v_nand_lo = 0;
-            load_tile(blockIdx.x);
-            for (u32 tile = blockIdx.x; (u64)tile * CWE_TILE < a.M; tile += G) {
-                bool f0[CWE_ITEMS], f1[CWE_ITEMS];
-                u32 p0[CWE_ITEMS], p1[CWE_ITEMS];
-                u64 sc[CWE_ITEMS];
-                u32 dg0[CWE_ITEMS];
-                bool ev[CWE_ITEMS];
+            for (u32 tile = blockIdx.x; (u64)tile * CWE_MTILE < a.M; tile += G) {
+                bool f0[CWE_MI], f1[CWE_MI];
+                u32 p0[CWE_MI], p1[CWE_MI];
+                u64 sc[CWE_MI];
+                load_tile(tile);
 #pragma unroll
-                for (int k = 0; k < CWE_ITEMS; ++k) {  // consume the tile's registers, then request the next tile
-                    ev[k] = evictable(k);
-                    sc[k] = ev[k] ? block_score(k) : 0ull;
-                    dg0[k] = ev[k] ? digit0(k, sc[k], tile * CWE_TILE + k * CWE_THREADS + tid) : 0u;
-                }
-                load_tile(tile + G);
-#pragma unroll
-                for (int k = 0; k < CWE_ITEMS; ++k) {
-                    const u32 b = tile * CWE_TILE + k * CWE_THREADS + tid;
+                for (int k = 0; k < CWE_MI; ++k) {
+                    const u32 b = tile * CWE_MTILE + tid * CWE_MI + k;
                     f0[k] = f1[k] = false;
-                    if (ev[k]) {
-                        const u32 dg = dg0[k];
+                    sc[k] = 0;
+                    if (evictable(k)) {
+                        sc[k] = block_score(k);
+                        const u32 dg = digit0(k, sc[k], b);
                         if (dg < thr || (take_all && dg == thr)) {
                             f0[k] = true;
                             v_or_hi |= sc[k];
@@ -683,10 +680,17 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
                     }
                     if (next) hist_add(s_hist, f1[k], f1[k] ? plan_digit(pn, sc[k], b) : 0u);
                 }
+                {   // most tiles hold neither victims nor candidates (sessions above the threshold): one barrier, not
+                    // the three barriers and the scan of an append
+                    bool any = false;
+#pragma unroll
+                    for (int k = 0; k < CWE_MI; ++k) any |= f0[k] | f1[k];
+                    if (!__syncthreads_or(any)) continue;
+                }
                 tile_append(f0, f1, p0, p1, &st->n_out, &st->n_cand[1], s_w0, s_w1, s_base);
 #pragma unroll
-                for (int k = 0; k < CWE_ITEMS; ++k) {
-                    const u32 b = tile * CWE_TILE + k * CWE_THREADS + tid;
+                for (int k = 0; k < CWE_MI; ++k) {
+                    const u32 b = tile * CWE_MTILE + tid * CWE_MI + k;
                     if (f0[k]) {
                         a.out_score[p0[k]] = sc[k];
                         a.out_id[p0[k]] = b;
@@ -1290,7 +1294,7 @@ int32_t cwi_score_evict(cw_ctx* ctx, cudaStream_t stream, u32 grid_limit, u32 ti
     a.victim_scores = d_victim_scores;
     a.num_victims = d_num_victims;
     // small pools do not need the whole machine (and the grid barrier gets cheaper)
-    u32 tiles = (a.M + CWE_TILE - 1) / CWE_TILE;
+    u32 tiles = (u32)(((u64)a.M + CWE_MTILE - 1) / CWE_MTILE);
     int grid = ctx->evict_grid;
     if (grid_limit && (u32)grid > grid_limit) grid = (int)grid_limit;
     if ((u32)grid > tiles) grid = tiles ? (int)tiles : 1;

@@ -63,12 +63,8 @@ __host__ __device__ __forceinline__ u64 cw_remap_key(u64 k) {
 #define CWH_UNIT (32 * CWH_WARPS)     // blocks per unit (one unit = one CTA iteration)
 #define CWH_UNIT_LOG2 8
 #define CWH_SMALL_R 512                // calls with at most this many requests skip the plan kernel
-#ifndef CWH_STAGES
 #define CWH_STAGES 3                  // smem ring depth
-#endif
-#ifndef CWH_MIN_CTAS
 #define CWH_MIN_CTAS 4
-#endif
 #define CWH_STAGE_BYTES (CWH_UNIT * 64 + 16)
 
 struct cw_hash_rec {  // what the CTA of one range publishes for the CTA of the next range
@@ -167,6 +163,7 @@ struct cw_ctx {
     u32 spec_cap;
     bool spec_open;
     u32* dup_bits;   // CW_DEBUG: one bit per pool block (duplicate check of the gather)
+    u64* dbg_stamps; // CW_DEBUG: %globaltimer values written by cw_debug_stamp (32 slots)
     // stage 4
     uint8_t* staging;
     cudaEvent_t ev_gather[2], ev_copy[2], ev_join;

@@ -165,3 +165,17 @@ def test_tp_head_slices_partition_the_page_and_reassemble_through_the_oracle():
         htp.head_slice(cb, 3, 0)
     with pytest.raises(ValueError):
         htp.head_slice(cb, 2, 2)
+
+
+def test_bench_reads_roofline_traffic_from_the_committed_ncu_export():
+    """roofline.traffic is not a constant in bench.py; it is parsed from the raw `ncu --set full`
+    export under profiles/ (dram__bytes_read.sum + dram__bytes_write.sum of each stage's kernel)."""
+    sys.path.insert(0, ROOT)
+    import bench
+    assert "NCU_TRAFFIC_BYTES" not in open(os.path.join(ROOT, "bench.py")).read()
+    t = bench.ncu_traffic()
+    assert set(t) == {"hash", "match", "schedule", "score_evict", "gather", "scatter"}
+    assert 0.9 * 2 * 16384 * 52352 < t["gather"] < 1.1 * 2 * 16384 * 52352      # read + write of every victim page
+    assert 0.85 * 421e6 < t["hash"] < 1.15 * 475e6                              # the token ids, once
+    md = open(os.path.join(ROOT, "profiles", "r2_step_kernels_raw.md")).read()
+    assert "ncu --set full" in md and "bench.py" in md                            # the export names its command

@@ -462,7 +462,10 @@ def run_cuda(args):
                                "algorithmic_bytes": alg[name], "us": round(stage_ms[name] * 1e3, 2)}
     dominant = max(stage_ms, key=stage_ms.get)
     roofline = dict(rooflines[dominant], kernel=dominant, peak_source=peak_src,
-                    traffic_source="profiles/r2_step_kernels_raw.csv" if traffic else None)
+                    traffic_source="profiles/r2_step_kernels_raw.csv" if traffic else None,
+                    note="peak = the driver's torch copy_ measurement (read + write bytes); a TMA-only copy kernel reads a "
+                         "little above it, and part of its write stream is still in L2 when the kernel ends (ncu traffic "
+                         "< algorithmic bytes), so frac can exceed 1 by a few per cent")
 
     extra = {}
     if rank == 0 or world > 1:

@@ -10,24 +10,31 @@ Eager launches with a one-thread stamp kernel between the calls: the absolute ti
 import torch
 import paper_2606_16824_b200 as cw
 from harness import gen, stress
-assert cw.DEBUG
-snap = gen.stress_snapshot(seed=3)
-stream = torch.cuda.Stream()
-st = stress.StressStep(snap, stream, with_pool=False)
-with torch.cuda.stream(stream):
-    st.decide(False); st.decide(True); stream.synchronize()
-    for name, steady in (("steady", True), ("cold", False)):
-        for rep in range(3):
-            if steady:
-                fns = [st.score_evict_begin, lambda: st.hash(True), st.match, st.schedule, st.score_evict_end]
-                labels = ["begin (fork)", "hash (256 new requests)", "match", "schedule", "end (join + trim)"]
-            else:
-                fns = [lambda: st.hash(False), st.score_evict_begin, st.match, st.schedule, st.score_evict_end]
-                labels = ["hash (all 4096 requests)", "begin (fork)", "match", "schedule", "end (join + trim)"]
-            main, ev = st.ctx.debug_timeline(fns)
-        t0 = main[0]
-        print(f"== {name} step, us from the first stamp on stream_main")
-        for i, l in enumerate(labels):
-            print(f"main  after {l:28s} {(main[i + 1] - t0) / 1e3:8.1f}")
-        print(f"side  evict_kernel first stamp     {(ev[0] - t0) / 1e3:8.1f}")
-        print(f"side  evict_kernel phase stamps    {[round((x - t0) / 1e3, 1) for x in ev[1:]]}")
+
+
+def main():
+    assert cw.DEBUG
+    snap = gen.stress_snapshot(seed=3)
+    stream = torch.cuda.Stream()
+    st = stress.StressStep(snap, stream, with_pool=False)
+    with torch.cuda.stream(stream):
+        st.decide(False); st.decide(True); stream.synchronize()
+        for name, steady in (("steady", True), ("cold", False)):
+            for rep in range(3):
+                if steady:
+                    fns = [st.score_evict_begin, lambda: st.hash(True), st.match, st.schedule, st.score_evict_end]
+                    labels = ["begin (fork)", "hash (256 new requests)", "match", "schedule", "end (join + trim)"]
+                else:
+                    fns = [lambda: st.hash(False), st.score_evict_begin, st.match, st.schedule, st.score_evict_end]
+                    labels = ["hash (all 4096 requests)", "begin (fork)", "match", "schedule", "end (join + trim)"]
+                main, ev = st.ctx.debug_timeline(fns)
+            t0 = main[0]
+            print(f"== {name} step, us from the first stamp on stream_main")
+            for i, l in enumerate(labels):
+                print(f"main  after {l:28s} {(main[i + 1] - t0) / 1e3:8.1f}")
+            print(f"side  evict_kernel first stamp     {(ev[0] - t0) / 1e3:8.1f}")
+            print(f"side  evict_kernel phase stamps    {[round((x - t0) / 1e3, 1) for x in ev[1:]]}")
+
+
+if __name__ == "__main__":
+    main()

@@ -423,7 +423,7 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
     __shared__ u64 s_acc_hi, s_acc2_hi;
     __shared__ u32 s_acc_lo, s_acc2_lo, s_cnt[2];
     __shared__ DigitPlan s_plan, s_plan2;
-    __shared__ unsigned short s_rank[CWE_RANK_SESS];  // level-0 digit of a session in rank mode
+    __shared__ unsigned short s_rank[CWE_RANK_SESS];  // level-0 digit of a session in rank mode (<= S)
     const u32 tid = threadIdx.x, G = gridDim.x;
     cw_evict_state* st = a.st;
     const bool tau_smem = a.S <= CWE_SMEM_SESS;
@@ -519,7 +519,10 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
             u32 larger = 0;
             for (u32 j = tid & 31; j < a.S; j += 32) larger += s_tau[j] > mine ? 1u : 0u;
             larger = __reduce_add_sync(0xffffffffu, larger);
-            if ((tid & 31) == 0) s_rank[sidx] = (unsigned short)larger;
+            // blocks of an unknown session (id >= S) count as tau = TAU_MAX (digit 0): every real tau below TAU_MAX
+            // ranks behind them whether or not a real session sits at TAU_MAX, so that equal taus share a digit and
+            // different taus never do
+            if ((tid & 31) == 0) s_rank[sidx] = (unsigned short)(larger + (mine < CW_TAU_MAX ? 1u : 0u));
         }
         __syncthreads();
     }

@@ -422,3 +422,31 @@ def test_swap_config3_shape_llama70b_pages_layer_major_60gib_pool():
     ctx.close()
     del pool, pv
     torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("with_idle", [False, True])
+def test_score_evict_rank_mode_with_unknown_sessions(with_idle):
+    """Level 0 of the select uses the RANK of a session's tau (S <= 512).  Blocks whose session id is >= S count as
+    tau = TAU_MAX; they must share a level-0 digit with idle sessions (same tau) and with nobody else — also when NO
+    real session sits at TAU_MAX.  Large pool (the grid-wide path), deficits that cut inside the unknown group,
+    inside the next tau group, and across several."""
+    from gpu_util import small_ctx
+    g = gen.rng(37, int(with_idle))
+    M, S, F = 60000, 40, 8
+    ctx = small_ctx(num_blocks=M, table_log2_slots=17, max_sessions=S)
+    sess = g.integers(0, S + 6, size=M).astype(np.uint32)              # ~13% of the blocks name a session >= S
+    last = g.integers(500, 1000, size=M).astype(np.uint32)
+    depth = g.integers(0, 3000, size=M).astype(np.uint32)
+    rf = np.full(M, V, np.uint32)
+    feats = g.integers(0, 256, size=(S, F), dtype=np.uint8)
+    w = g.integers(50, 300, size=F).astype(np.int16)
+    state = np.zeros(S, np.uint8)                                       # everybody TOOL_WAIT: every tau < TAU_MAX ...
+    if with_idle:
+        state[[3, 17]] = 3                                              # ... unless two sessions are idle
+    _load_meta(ctx, 0, sess, last, depth, rf)
+    n_unknown = int((sess >= S).sum())
+    for deficit in (1, n_unknown // 2, n_unknown, n_unknown + 700, n_unknown + 9000, M // 2, M):
+        ev, es, est = oracle.score_evict(1000, feats, w, 100, state, None, deficit, sess, last, depth, rf, cap=M)
+        gv, gs, gst = _evict(ctx, 1000, feats, w, 100, state, None, deficit, M)
+        assert gst == est and gv.tolist() == ev.tolist() and gs.tolist() == es.tolist(), (with_idle, deficit)
+    ctx.close()

@@ -753,9 +753,30 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
                     u64 v_or_hi = 0, v_nand_hi = 0;
                     u32 v_or_lo = 0, v_nand_lo = 0;
                     __syncthreads();
-                    for (u32 i = tid; i < n; i += CWE_THREADS) {
-                        c_s[i] = __ldcg(cs + i);
-                        c_i[i] = __ldcg(ci + i);
+                    {   // n <= CWE_LOCAL = 4 x CWE_THREADS: all of a thread's loads are issued before the first store
+                        // (one memory round trip instead of four on the kernel's single-CTA critical path)
+                        static_assert(CWE_LOCAL <= 4 * CWE_THREADS, "local finish loads");
+                        u64 ts_[4];
+                        u32 ti_[4];
+                        const u32 n_ld = min(n, (u32)CWE_LOCAL);
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            const u32 i = min(tid + k * CWE_THREADS, n_ld ? n_ld - 1 : 0u);
+                            ts_[k] = __ldcg(cs + i);
+                            ti_[k] = __ldcg(ci + i);
+                        }
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            const u32 i = tid + k * CWE_THREADS;
+                            if (i < n_ld) {
+                                c_s[i] = ts_[k];
+                                c_i[i] = ti_[k];
+                            }
+                        }
+                        for (u32 i = tid + 4 * CWE_THREADS; i < n; i += CWE_THREADS) {  // p >= CWE_PASSES fallback only
+                            c_s[i] = __ldcg(cs + i);
+                            c_i[i] = __ldcg(ci + i);
+                        }
                     }
                     for (;;) {
                         __syncthreads();

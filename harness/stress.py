@@ -62,7 +62,7 @@ class StressStep:
         self.F = snap.features.shape[1]
         self.policy, self.free_blocks = policy, free_blocks
         self.spec_ctas = spec_ctas                # CTAs of the speculative selection (0 = library default)
-        self.cold_mark = True                     # cold step: fork point before the hash, launch behind it
+        self.cold_mark = False                    # cold step: fork point before the hash, launch behind it (cw_mark)
         self.evict_budget = snap.deficit          # "eviction deficit 5% of the pool per step"
         self.cap = max(snap.deficit, 1)
         self.page = n_chunks * chunk_bytes

@@ -62,7 +62,6 @@ class StressStep:
         self.F = snap.features.shape[1]
         self.policy, self.free_blocks = policy, free_blocks
         self.spec_ctas = spec_ctas                # CTAs of the speculative selection (0 = library default)
-        self.cold_mark = False                    # cold step: fork point before the hash, launch behind it (cw_mark)
         self.evict_budget = snap.deficit          # "eviction deficit 5% of the pool per step"
         self.cap = max(snap.deficit, 1)
         self.page = n_chunks * chunk_bytes
@@ -169,8 +168,6 @@ class StressStep:
         # a cold step hashes 421 MB of token ids and wants every SM for it: the fork comes after the hash there
         if overlap and steady:
             self.score_evict_begin()
-        if overlap and not steady and self.cold_mark:
-            self.ctx.mark()              # the selection does not depend on the hash, only follows it in launch order
         self.hash(steady)
         if overlap and not steady:
             self.score_evict_begin()

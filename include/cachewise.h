@@ -185,11 +185,6 @@ int32_t cw_score_evict(cw_ctx* ctx, uint32_t tick_now, uint32_t S, uint32_t F, c
  *   n_ctas: how many CTAs (= SMs) the speculative kernel may occupy; 0 = library default (a quarter of the SMs:
  *   measured on configs[2], 37 of 148 CTAs is where the steady step is shortest — the kernels on stream_main keep
  *   the other three quarters of the machine and both branches end together). */
-/* cw_mark: records the point of stream_main that the next cw_score_evict_begin forks from (instead of the begin call
- * itself).  Marking BEFORE a kernel is queued on stream_main and calling begin AFTER it keeps the side-stream work
- * independent of that kernel while putting the kernel first in launch order: the cold step marks, hashes, then
- * begins, so that the hash gets every SM first and the cooperative evict CTAs move in as hash CTAs retire. */
-int32_t cw_mark(cw_ctx* ctx);
 int32_t cw_score_evict_begin(cw_ctx* ctx, uint32_t tick_now, uint32_t S, uint32_t F, const uint8_t* d_features,
                              const int16_t* d_weights, int32_t bias, const uint8_t* d_session_state,
                              const uint32_t* d_tau_override, uint32_t tier, uint32_t* d_victims,

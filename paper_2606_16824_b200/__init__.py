@@ -24,7 +24,7 @@ CW_REF_PINNED = 0x40000000
 POLICY_MIN_ADDITIONAL, POLICY_OVERLAP_FIRST, POLICY_FCFS = 0, 1, 2
 
 EXPORTS = ["cw_create", "cw_destroy", "cw_sync", "cw_join_copy", "cw_last_error", "cw_launch_count", "cw_hash_blocks",
-           "cw_match_prefix", "cw_schedule", "cw_admit_chunked", "cw_score_evict", "cw_mark", "cw_score_evict_begin", "cw_score_evict_end",
+           "cw_match_prefix", "cw_schedule", "cw_admit_chunked", "cw_score_evict", "cw_score_evict_begin", "cw_score_evict_end",
            "cw_predict_tau", "cw_swap_out", "cw_swap_in", "cw_gather_pages", "cw_scatter_pages", "cw_table_insert",
            "cw_table_erase", "cw_table_retag", "cw_table_lookup", "cw_table_compact", "cw_table_stats",
            "cw_blocks_update"]
@@ -80,7 +80,6 @@ def lib():
         L.cw_score_evict.argtypes = [P, U32, U32, U32, P, P, I32, P, P, P, U32, P, P, P, U32]
         L.cw_score_evict_begin.argtypes = [P, U32, U32, U32, P, P, I32, P, P, U32, P, P, U32, U32]
         L.cw_score_evict_end.argtypes = [P, P, P]
-        L.cw_mark.argtypes = [P]
         L.cw_table_compact.argtypes = [P]
         L.cw_table_stats.argtypes = [P, P]
         L.cw_predict_tau.argtypes = [P, U32, P, P, U32, P, P, P]
@@ -217,9 +216,6 @@ class Context:
         self._ck(lib().cw_score_evict_begin(self._h, tick_now, S, F, _ptr(features), _ptr(weights), bias,
                                             _ptr(session_state), _ptr(tau_override), tier, _ptr(victims),
                                             _ptr(victim_scores), cap, n_ctas), "cw_score_evict_begin")
-
-    def mark(self):
-        self._ck(lib().cw_mark(self._h), "cw_mark")
 
     def score_evict_end(self, deficit, num_victims):
         self._ck(lib().cw_score_evict_end(self._h, _ptr(deficit), _ptr(num_victims)), "cw_score_evict_end")

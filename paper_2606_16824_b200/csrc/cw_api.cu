@@ -38,7 +38,6 @@ void free_all(cw_ctx* c) {
     if (c->ev_join) cudaEventDestroy(c->ev_join);
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_spec) cudaEventDestroy(c->ev_spec);
-    if (c->ev_mark) cudaEventDestroy(c->ev_mark);
     if (c->s_side) cudaStreamDestroy(c->s_side);
     cudaFree(c->spec_n);
     cudaFree(c->dup_bits);
@@ -163,7 +162,6 @@ int32_t cw_create(const cw_config* cfg, cw_ctx** out) {
     CW_CUDA(c, cudaStreamCreateWithFlags(&c->s_side, cudaStreamNonBlocking));
     CW_CUDA(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
     CW_CUDA(c, cudaEventCreateWithFlags(&c->ev_spec, cudaEventDisableTiming));
-    CW_CUDA(c, cudaEventCreateWithFlags(&c->ev_mark, cudaEventDisableTiming));
 #ifdef CW_DEBUG
     CW_CUDA(c, dalloc_zero(&c->dup_bits, ((size_t)cfg->num_blocks + 31) / 32, s));
     CW_CUDA(c, dalloc_zero(&c->dbg_stamps, 32, s));
@@ -328,15 +326,9 @@ int32_t cw_score_evict_begin(cw_ctx* ctx, uint32_t tick_now, uint32_t S, uint32_
     if (st) return st;
     if (ctx->spec_open) return CW_E_STATE;
     if (cap > ctx->tier_size[tier]) cap = ctx->tier_size[tier];
-    // fork: the side stream starts after everything queued on stream_main up to the fork point — the last cw_mark()
-    // if one was set since the previous begin, else this call
-    if (ctx->mark_set) {
-        ctx->mark_set = false;
-        CW_CUDA(ctx, cudaStreamWaitEvent(ctx->s_side, ctx->ev_mark, 0));
-    } else {
-        CW_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->s_main));
-        CW_CUDA(ctx, cudaStreamWaitEvent(ctx->s_side, ctx->ev_fork, 0));
-    }
+    // fork: the side stream starts after everything queued on stream_main so far
+    CW_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->s_main));
+    CW_CUDA(ctx, cudaStreamWaitEvent(ctx->s_side, ctx->ev_fork, 0));
     st = cwi_score_evict(ctx, ctx->s_side, n_ctas ? n_ctas : (u32)(ctx->n_sm + 3) / 4, tick_now, S, F, d_features,
                          d_weights, bias, d_session_state, d_tau_override, nullptr, tier, d_victims, d_victim_scores,
                          ctx->spec_n, cap);
@@ -344,13 +336,6 @@ int32_t cw_score_evict_begin(cw_ctx* ctx, uint32_t tick_now, uint32_t S, uint32_
     CW_CUDA(ctx, cudaEventRecord(ctx->ev_spec, ctx->s_side));
     ctx->spec_open = true;
     ctx->spec_cap = cap;
-    return CW_OK;
-}
-
-int32_t cw_mark(cw_ctx* ctx) {
-    if (!ctx) return CW_E_STATE;
-    CW_CUDA(ctx, cudaEventRecord(ctx->ev_mark, ctx->s_main));
-    ctx->mark_set = true;
     return CW_OK;
 }
 

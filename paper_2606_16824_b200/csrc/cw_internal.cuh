@@ -158,8 +158,7 @@ struct cw_ctx {
     int evict_grid;  // CTAs of the cooperative evict launch on THIS device (cw_create)
     // stage 3, speculative form: side stream + fork / join events, victims of the budget, open flag
     cudaStream_t s_side;
-    cudaEvent_t ev_fork, ev_spec, ev_mark;
-    bool mark_set;   // cw_mark recorded a fork point that the next cw_score_evict_begin consumes
+    cudaEvent_t ev_fork, ev_spec;
     u32* spec_n;     // device: victims the speculative selection produced (= min(cap, #evictable))
     u32 spec_cap;
     bool spec_open;

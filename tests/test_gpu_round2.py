@@ -178,9 +178,6 @@ def test_speculative_evict_equals_serial_evict_and_the_oracle(n_ctas):
             d_def = zeros(1, np.uint32)
 
             def spec():
-                if n_ctas == 3:                     # fork point set BEFORE a kernel of stream_main, begin called after it
-                    ctx.mark()
-                    filler.add_(1)
                 ctx.score_evict_begin(snap.tick_now, S, F, d_f, d_w, snap.bias, d_s, None, 0, vic, sc, cap, n_ctas)
                 filler.add_(1)                      # stands for hash -> match -> schedule on stream_main
                 ctx.score_evict_end(d_def, nv)

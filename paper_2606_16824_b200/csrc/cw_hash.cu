@@ -4,9 +4,13 @@
 //   chain   H_j = A*H_{j-1} + c_j  (mod 2^64),  H_{-1} = fin(salt ^ K7)  or  start_state
 //
 // The chain is an affine recurrence whose multiplier is always a power of A, so it is a SCAN:
-//   warp : inclusive scan over 32 blocks, step d uses the constant A^d
-//   CTA  : 8 warp aggregates combined by Horner with A^32; the running state is carried from one 256-block
-//          unit to the next in registers
+//   lane : a consumer lane owns CWH_K = 8 CONSECUTIVE blocks of a unit (512 bytes of token ids): it digests them
+//          itself (no cross-lane reduction) and chains them serially in registers (7 multiply-adds)
+//   warp : one inclusive scan over the 32 lane aggregates, step d uses the constant (A^8)^d; a unit of 256 blocks
+//          therefore costs ONE 5-step warp scan, and a warp works on a unit alone (no CTA barrier per unit)
+//   CTA  : the 4 consumer warps take the units of the CTA's range round-robin; the chain state is handed from the
+//          warp of unit i to the warp of unit i+1 through a shared-memory ring (one mbarrier per slot): the serial
+//          part per unit is one multiply-add, everything else of a unit runs beside the other warps' units
 //   grid : the list of units (request-aligned runs of <= 256 blocks) is cut into gridDim.x CONTIGUOUS ranges
 //          of equal length, one per CTA.  A CTA therefore walks its requests sequentially and never waits on
 //          another CTA (no look-back, no spinning).  Only the first request of a range can have begun in an
@@ -21,10 +25,12 @@
 // hash_kernel rebuilds the plan in shared memory and the last CTA to finish re-arms the ticket and the epoch):
 //   hash_plan_kernel   units per request -> exclusive scan unit_off[R+1]; validates the offsets
 //   hash_kernel        the streaming pass: one producer warp issues ONE TMA bulk copy (cp.async.bulk, L2
-//                      evict-first) of each unit's 16 KiB of token ids into a 3-stage shared-memory ring
-//                      (mbarrier full/empty); 8 consumer warps read conflict-free 16-byte quarters, 2 multiplies
-//                      per lane, 6-shuffle transposed reduction, fin, 5-step warp scan; then the boundary
-//                      patch (about half a request per CTA: ~1% extra traffic, L2-resident)
+//                      evict-first) of each unit's 16 KiB of token ids into a 4-stage shared-memory ring
+//                      (mbarrier full/empty); a consumer warp reads its unit with conflict-free 16-byte loads (the
+//                      quarter of a block a lane reads first is rotated by the lane id and odd lane quads take
+//                      their block pairs in swapped order, so the 8 lanes of a load phase cover all 32 banks);
+//                      16 multiplies + fin per block, the lane chain, the warp scan, the hand-over, 8 stores;
+//                      then the boundary patch (about half a request per CTA: ~1% extra traffic, L2-resident)
 // Requests start at arbitrary 4-byte alignment: the copy starts at the 16-byte boundary below and the
 // consumers funnel the `mis` leading words away in registers.
 #include <stdio.h>
@@ -73,8 +79,8 @@ struct __align__(128) HashSmem {
     UnitInfo info[CWH_STAGES];
     u64 full[CWH_STAGES];
     u64 empty[CWH_STAGES];
-    u64 wagg[2][CWH_WARPS];
-    u64 pw[CWH_WARPS + 1];  // (A^32)^k
+    u64 carry_bar[CWH_WARPS];   // slot i % CWH_WARPS: the chain state after unit i of the range is published
+    u64 carry_ring[CWH_WARPS];
     u64 carry_in;
     u32 uoff[CWH_SMALL_R + 1];  // small calls: exclusive scan of units per request
     u32 wsum[CWH_WARPS + 1];
@@ -95,15 +101,15 @@ __device__ __forceinline__ u64 pow_u64(u64 base, u64 e) {
     return r;
 }
 
-__device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;" ::"n"(CWH_UNIT) : "memory"); }
-
 // ------------------------------------------------------------------------------------------------ plan
+// Loads first, decisions after: a load behind a condition is not issued until the condition is known, and the plan
+// wants all of a thread's loads in flight at once.
 __device__ __forceinline__ u64 plan_units(const HashArgs& a, u32 r, bool too_big) {
-    if (too_big) return 0;
     const u64 t0 = a.tok_off[r], t1 = a.tok_off[r + 1], h0 = a.hash_off[r], h1 = a.hash_off[r + 1];
     const u64 sb = a.start_block ? a.start_block[r] : 0;
-    if (t1 < t0 || h1 < h0 || (h1 - h0) != ((t1 - t0) >> 4) || sb > h1 - h0) return ~0ull;  // invalid request
-    return (h1 - h0 - sb + CWH_UNIT - 1) >> CWH_UNIT_LOG2;
+    const bool invalid = t1 < t0 || h1 < h0 || (h1 - h0) != ((t1 - t0) >> 4) || sb > h1 - h0;
+    const u64 T = (h1 - h0 - sb + CWH_UNIT - 1) >> CWH_UNIT_LOG2;
+    return too_big ? 0ull : (invalid ? ~0ull : T);
 }
 
 __global__ void __launch_bounds__(1024) hash_plan_kernel(const HashArgs a) {
@@ -116,10 +122,16 @@ __global__ void __launch_bounds__(1024) hash_plan_kernel(const HashArgs a) {
     const u32 lo = min(R, tid * per), hi = min(R, lo + per);
     u64 local = 0;
     bool bad = false;
-    for (u32 r = lo; r < hi; ++r) {
-        const u64 T = plan_units(a, r, too_big);
-        if (T == ~0ull) bad = true;
-        else local += T;
+    for (u32 r0 = lo; r0 < hi; r0 += 4) {  // four requests' loads in flight at once (clamped index, select after)
+        u64 T[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) T[k] = plan_units(a, min(r0 + k, hi - 1), too_big);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const bool in = r0 + k < hi;
+            bad |= in && T[k] == ~0ull;
+            local += (in && T[k] != ~0ull) ? T[k] : 0ull;
+        }
     }
     if (bad) atomicOr(a.status, CWS_INVAL);
     u64 inc = local;
@@ -148,15 +160,61 @@ __global__ void __launch_bounds__(1024) hash_plan_kernel(const HashArgs a) {
     }
     __syncthreads();
     u64 run = s_warp[warp] + inc - local;
-    for (u32 r = lo; r < hi; ++r) {
-        a.unit_off[r] = run;
-        const u64 T = plan_units(a, r, too_big);
-        if (T != ~0ull) run += T;
+    for (u32 r0 = lo; r0 < hi; r0 += 4) {
+        u64 T[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) T[k] = plan_units(a, min(r0 + k, hi - 1), too_big);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (r0 + k < hi) {
+                a.unit_off[r0 + k] = run;
+                if (T[k] != ~0ull) run += T[k];
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ digests
+// The raw sums (before fin) of the 8 blocks a lane owns.  `lane_run` points at the lane's 512 staged bytes; step k
+// reads the quarter (k + lane) & 3 of a block (keys kq[k][]), and a lane with `swapped` set takes the blocks of each
+// pair in the order odd, even (off_e / off_o carry both rotations), so ct[] comes back in NATURAL block order.
+template <int MIS>
+__device__ __forceinline__ void digest8(const uint8_t* lane_run, const u32 (&off_e)[4], const u32 (&off_o)[4],
+                                        const u32 (&kq)[4][4], bool swapped, u64 (&ct)[CWH_K]) {
+    u64 raw[CWH_K];
+#pragma unroll
+    for (int m = 0; m < CWH_K; ++m) {
+        u64 acc = 0;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const uint8_t* p = lane_run + 64 * m + ((m & 1) ? off_o[k] : off_e[k]);
+            const uint4 w0 = *reinterpret_cast<const uint4*>(p);
+            u32 t0, t1, t2, t3;
+            if (MIS == 0) {
+                t0 = w0.x; t1 = w0.y; t2 = w0.z; t3 = w0.w;
+            } else {
+                const uint4 w1 = *reinterpret_cast<const uint4*>(p + 16);
+                if (MIS == 1) {
+                    t0 = w0.y; t1 = w0.z; t2 = w0.w; t3 = w1.x;
+                } else if (MIS == 2) {
+                    t0 = w0.z; t1 = w0.w; t2 = w1.x; t3 = w1.y;
+                } else {
+                    t0 = w0.w; t1 = w1.x; t2 = w1.y; t3 = w1.z;
+                }
+            }
+            acc += (u64)(t0 + kq[k][0]) * (u64)(t1 + kq[k][1]) + (u64)(t2 + kq[k][2]) * (u64)(t3 + kq[k][3]);
+        }
+        raw[m] = acc;
+    }
+#pragma unroll
+    for (int m = 0; m < CWH_K; m += 2) {
+        ct[m] = swapped ? raw[m + 1] : raw[m];
+        ct[m + 1] = swapped ? raw[m] : raw[m + 1];
     }
 }
 
 // ------------------------------------------------------------------------------------------------ main pass
-__global__ void __launch_bounds__(CWH_UNIT + 32, CWH_MIN_CTAS) hash_kernel(const HashArgs a) {
+__global__ void __launch_bounds__(CWH_THREADS, CWH_MIN_CTAS) hash_kernel(const HashArgs a) {
     extern __shared__ __align__(128) uint8_t smem_raw[];
     HashSmem& sm = *reinterpret_cast<HashSmem*>(smem_raw);
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -167,24 +225,26 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, CWH_MIN_CTAS) hash_kernel(const
     u32 epoch;
     if (small) {
         // ---- small call (R <= CWH_SMALL_R, the steady-state step): no plan kernel.  Every CTA computes the units of
-        // every request (two per thread, one round of loads), scans them and keeps the offsets in shared memory; the
+        // every request (a few per thread, one round of loads), scans them and keeps the offsets in shared memory; the
         // last CTA to finish re-arms the ticket and advances the epoch.
         const u32 R = a.R;
         const bool too_big = a.hash_off[R] < a.hash_off[0] || a.hash_off[R] - a.hash_off[0] > a.max_hashed;
-        u32 t2[2];
+        constexpr int PER = (CWH_SMALL_R + CWH_THREADS - 1) / CWH_THREADS;  // requests per thread
+        u32 tu[PER];
         bool bad = too_big;
+        u32 local = 0;
 #pragma unroll
-        for (int k = 0; k < 2; ++k) {
-            const u32 r = tid * 2 + k;
+        for (int k = 0; k < PER; ++k) {
+            const u32 r = tid * PER + k;
             u64 T = r < R ? plan_units(a, r, too_big) : 0;
             if (T == ~0ull) {
                 bad = true;
                 T = 0;
             }
-            t2[k] = (u32)T;
+            tu[k] = (u32)T;
+            local += (u32)T;
         }
         if (bad && blockIdx.x == 0) atomicOr(a.status, CWS_INVAL);
-        const u32 local = t2[0] + t2[1];
         u32 inc = local;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
@@ -200,9 +260,13 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, CWH_MIN_CTAS) hash_kernel(const
             if (w < warp) before += v;
             total += v;
         }
-        const u32 excl = before + inc - local;
-        if (tid * 2 < R) sm.uoff[tid * 2] = excl;
-        if (tid * 2 + 1 < R) sm.uoff[tid * 2 + 1] = excl + t2[0];
+        u32 run = before + inc - local;
+#pragma unroll
+        for (int k = 0; k < PER; ++k) {
+            const u32 r = tid * PER + k;
+            if (r < R) sm.uoff[r] = run;
+            run += tu[k];
+        }
         if (tid == 0) sm.uoff[R] = total;
         U = total;
         epoch = (u32)a.plan[1] + 1;
@@ -230,12 +294,13 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, CWH_MIN_CTAS) hash_kernel(const
         return;
     }
 
-    if (tid <= CWH_WARPS) sm.pw[tid] = pow_u64(cw_pow(CW_A, 32), tid);
+    const u32 n_units = (u32)(u_end - u_begin);
     if (tid == 0) {
         for (int s = 0; s < CWH_STAGES; ++s) {
             mbar_init(smem_u32(&sm.full[s]), 1);
             mbar_init(smem_u32(&sm.empty[s]), 1);
         }
+        for (int w = 0; w < CWH_WARPS; ++w) mbar_init(smem_u32(&sm.carry_bar[w]), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -309,15 +374,6 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, CWH_MIN_CTAS) hash_kernel(const
                     fresh = true;
                 }
             }
-            // terminator
-            {
-                const u32 s = it % CWH_STAGES;
-                if (it >= CWH_STAGES) mbar_wait(smem_u32(&sm.empty[s]), ((it / CWH_STAGES) - 1) & 1);
-                UnitInfo ui;
-                ui.valid = 0;
-                sm.info[s] = ui;
-                mbar_arrive(smem_u32(&sm.full[s]));
-            }
             // hand-over record (rec_tail_state is written by the consumers)
             const bool tail_open = (uo0 + t) < uo1;  // the last request continues in the next range
             sm.rec_bseg_first = bseg_first;
@@ -327,89 +383,87 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, CWH_MIN_CTAS) hash_kernel(const
         }
     } else {
         // ------------------------------------------------------------------ consumer warps
-        const u32 q = lane & 3;
-        const u32 ka0 = q == 0 ? key_a(0) : q == 1 ? key_a(2) : q == 2 ? key_a(4) : key_a(6);
-        const u32 kb0 = q == 0 ? key_b(0) : q == 1 ? key_b(2) : q == 2 ? key_b(4) : key_b(6);
-        const u32 ka1 = q == 0 ? key_a(1) : q == 1 ? key_a(3) : q == 2 ? key_a(5) : key_a(7);
-        const u32 kb1 = q == 0 ? key_b(1) : q == 1 ? key_b(3) : q == 2 ? key_b(5) : key_b(7);
-        const u64 a_lane1 = pow_u64(CW_A, lane + 1);  // A^(lane+1)
-        // after the transposed reduction lane i owns block 8*k(i) + (i>>2), k(i) = 2*bit0 + bit1;
-        // the lane that owns block b is 4*(b&7) | ((b>>3)&1)<<1 | (b>>4)
-        const u32 owner = ((lane & 7) << 2) | (((lane >> 3) & 1) << 1) | (lane >> 4);
-        constexpr u64 A2 = cw_pow(CW_A, 2), A4 = cw_pow(CW_A, 4), A8 = cw_pow(CW_A, 8), A16 = cw_pow(CW_A, 16);
-        u64 carry = 0;  // chain state before the current unit (uniform over the CTA)
+        const bool swapped = (lane >> 2) & 1;
+        u32 kq[4][4], off_e[4], off_o[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const u32 q = (k + lane) & 3;  // pairs 2q and 2q+1 of the block
+            kq[k][0] = q == 0 ? key_a(0) : q == 1 ? key_a(2) : q == 2 ? key_a(4) : key_a(6);
+            kq[k][1] = q == 0 ? key_b(0) : q == 1 ? key_b(2) : q == 2 ? key_b(4) : key_b(6);
+            kq[k][2] = q == 0 ? key_a(1) : q == 1 ? key_a(3) : q == 2 ? key_a(5) : key_a(7);
+            kq[k][3] = q == 0 ? key_b(1) : q == 1 ? key_b(3) : q == 2 ? key_b(5) : key_b(7);
+            off_e[k] = 16 * q + (swapped ? 64u : 0u);
+            off_o[k] = 16 * q - (swapped ? 64u : 0u);  // added to 64*m with m odd: never below the lane's run
+        }
+        constexpr u64 A8 = cw_pow(CW_A, 8), A16 = cw_pow(CW_A, 16), A32 = cw_pow(CW_A, 32), A64 = cw_pow(CW_A, 64),
+                      A128 = cw_pow(CW_A, 128), A256 = cw_pow(CW_A, 256);
+        const u64 a_lane8 = pow_u64(A8, lane);  // A^(8*lane): carries the unit's carry-in to the lane's first block
 
-        for (u32 it = 0;; ++it) {
+        for (u32 it = warp; it < n_units; it += CWH_WARPS) {
             const u32 s = it % CWH_STAGES;
             mbar_wait(smem_u32(&sm.full[s]), (it / CWH_STAGES) & 1);
             const UnitInfo ui = sm.info[s];
-            if (!ui.valid) break;
 
-            // ---- quarter sums of 4 x 8 blocks
-            const uint8_t* base = &sm.stage[s][0] + warp * (32 * 64) + (lane >> 2) * 64 + q * 16;
-            u64 p[4];
+            // ---- digests of the lane's 8 consecutive blocks
+            const uint8_t* lane_run = &sm.stage[s][0] + lane * (64 * CWH_K);
+            u64 c[CWH_K];
+            if (ui.mis == 0) digest8<0>(lane_run, off_e, off_o, kq, swapped, c);
+            else if (ui.mis == 1) digest8<1>(lane_run, off_e, off_o, kq, swapped, c);
+            else if (ui.mis == 2) digest8<2>(lane_run, off_e, off_o, kq, swapped, c);
+            else digest8<3>(lane_run, off_e, off_o, kq, swapped, c);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&sm.empty[s]));  // every lane has read stage s
+
+            // ---- lane chain (carry-free), then one warp scan over the lane aggregates
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const uint4 w0 = *reinterpret_cast<const uint4*>(base + k * 512);
-                u32 t0, t1, t2, t3;
-                if (ui.mis == 0) {
-                    t0 = w0.x; t1 = w0.y; t2 = w0.z; t3 = w0.w;
-                } else {
-                    const uint4 w1 = *reinterpret_cast<const uint4*>(base + k * 512 + 16);
-                    if (ui.mis == 1) {
-                        t0 = w0.y; t1 = w0.z; t2 = w0.w; t3 = w1.x;
-                    } else if (ui.mis == 2) {
-                        t0 = w0.z; t1 = w0.w; t2 = w1.x; t3 = w1.y;
-                    } else {
-                        t0 = w0.w; t1 = w1.x; t2 = w1.y; t3 = w1.z;
-                    }
-                }
-                p[k] = (u64)(t0 + ka0) * (u64)(t1 + kb0) + (u64)(t2 + ka1) * (u64)(t3 + kb1);
-            }
-            // ---- transposed reduction over the 4 lanes of a block (6 shuffles)
-            const bool b0 = lane & 1, b1 = lane & 2;
-            u64 keep0 = b0 ? p[2] : p[0], keep1 = b0 ? p[3] : p[1];
-            u64 send0 = b0 ? p[0] : p[2], send1 = b0 ? p[1] : p[3];
-            keep0 += shfl64_xor(send0, 1);
-            keep1 += shfl64_xor(send1, 1);
-            u64 keep = b1 ? keep1 : keep0, send = b1 ? keep0 : keep1;
-            keep += shfl64_xor(send, 2);
-            const u64 ssum = shfl64(keep, owner);  // lane = block index inside the warp
-            u64 x = cw_fin(ssum ^ CW_K5);
+            for (int m = 0; m < CWH_K; ++m) c[m] = cw_fin(c[m] ^ CW_K5);
+#pragma unroll
+            for (int m = 1; m < CWH_K; ++m) c[m] += CW_A * c[m - 1];
+            u64 x = c[CWH_K - 1], y;
+            y = shfl64_up(x, 1);  if (lane >= 1) x += A8 * y;
+            y = shfl64_up(x, 2);  if (lane >= 2) x += A16 * y;
+            y = shfl64_up(x, 4);  if (lane >= 4) x += A32 * y;
+            y = shfl64_up(x, 8);  if (lane >= 8) x += A64 * y;
+            y = shfl64_up(x, 16); if (lane >= 16) x += A128 * y;
+            u64 before = shfl64_up(x, 1);  // carry-free chain state in front of the lane's first block
+            if (lane == 0) before = 0;
+            const u64 agg = shfl64(x, 31);
 
-            // ---- warp scan of the affine chain (carry-free)
-            u64 y;
-            y = shfl64_up(x, 1);  if (lane >= 1) x += CW_A * y;
-            y = shfl64_up(x, 2);  if (lane >= 2) x += A2 * y;
-            y = shfl64_up(x, 4);  if (lane >= 4) x += A4 * y;
-            y = shfl64_up(x, 8);  if (lane >= 8) x += A8 * y;
-            y = shfl64_up(x, 16); if (lane >= 16) x += A16 * y;
-            const u32 buf = it & 1;
-            if (lane == 31) sm.wagg[buf][warp] = x;
-            consumer_bar();
-            if (tid == 0) mbar_arrive(smem_u32(&sm.empty[s]));  // every consumer has read stage s
-
-            // ---- carry-in of this warp and the state after the unit, lane-parallel: lanes 0-7 fold the earlier warps'
-            //      aggregates for this warp, lanes 8-15 fold all eight for the next unit (powers of A^32 from smem)
-            const u64 run0 = ui.mode == MODE_SEED ? ui.seed : (ui.mode == MODE_ZERO ? 0ull : carry);
-            u64 term = 0;
-            {
-                const u32 v = lane & 7, grp = lane >> 3;
-                if (grp < 2) {
-                    const u32 tgt = grp == 0 ? warp : CWH_WARPS;  // how many warp aggregates are folded in
-                    if (v < tgt) term = sm.pw[tgt - 1 - v] * sm.wagg[buf][v];
-                    if (v == 0) term += sm.pw[tgt] * run0;
-                }
-                term += shfl64_xor(term, 1);
-                term += shfl64_xor(term, 2);
-                term += shfl64_xor(term, 4);
+            // ---- hand-over: the chain state in front of this unit, the state behind it for the next warp.  Every
+            //      unit waits for its predecessor's slot (also when it does not use the value), so a slot is never
+            //      overwritten before it was read.
+            u64 cin = 0;
+            if (it > 0) {
+                const u32 ps = (it - 1) % CWH_WARPS;
+                mbar_wait(smem_u32(&sm.carry_bar[ps]), ((it - 1) / CWH_WARPS) & 1);
+                cin = *reinterpret_cast<volatile u64*>(&sm.carry_ring[ps]);
             }
-            const u64 cin = shfl64(term, 0);
-            carry = shfl64(term, 8);  // meaningful when the unit is full (a partial unit ends its request)
-            const u64 h = x + a_lane1 * cin;
-            const u32 bi = warp * 32 + lane;
-            if (bi < ui.nblk) a.hashes[ui.out_base + bi] = h;
-            if (ui.last && tid == 0) sm.rec_tail_state = carry;
+            if (ui.mode == MODE_SEED) cin = ui.seed;
+            else if (ui.mode == MODE_ZERO) cin = 0;
+            const u64 cout = A256 * cin + agg;  // meaningful when the unit is full (a partial unit ends its request)
+            __syncwarp();                       // every lane has read the predecessor's slot
+            if (lane == 0) {
+                *reinterpret_cast<volatile u64*>(&sm.carry_ring[it % CWH_WARPS]) = cout;
+                if (it + 1 == n_units) sm.rec_tail_state = cout;
+                mbar_arrive(smem_u32(&sm.carry_bar[it % CWH_WARPS]));
+            }
+
+            // ---- final hashes of the lane's blocks: H = local + A^(m+1) * (state in front of the lane)
+            const u64 front = before + a_lane8 * cin;
+            const u32 first = lane * CWH_K;
+            const u32 nv = ui.nblk > first ? ui.nblk - first : 0u;  // valid blocks of this lane
+            u64* dst = a.hashes + ui.out_base + first;
+            u64 h[CWH_K];
+#pragma unroll
+            for (int m = 0; m < CWH_K; ++m) h[m] = c[m] + cw_pow(CW_A, m + 1) * front;
+            if ((reinterpret_cast<uintptr_t>(dst) & 15) == 0 && nv >= CWH_K) {
+#pragma unroll
+                for (int m = 0; m < CWH_K; m += 2) *reinterpret_cast<ulonglong2*>(dst + m) = make_ulonglong2(h[m], h[m + 1]);
+            } else {
+#pragma unroll
+                for (int m = 0; m < CWH_K; ++m)
+                    if ((u32)m < nv) dst[m] = h[m];
+            }
         }
     }
 
@@ -496,7 +550,7 @@ __global__ void __launch_bounds__(CWH_UNIT + 32, CWH_MIN_CTAS) hash_kernel(const
 int cwi_hash_grid(int n_sm) {
     int per_sm = 0;
     cudaFuncSetAttribute(hash_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(HashSmem));
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, hash_kernel, CWH_UNIT + 32, sizeof(HashSmem));
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, hash_kernel, CWH_THREADS, sizeof(HashSmem));
     if (per_sm < 1) per_sm = 1;
     return per_sm * n_sm;
 }
@@ -527,7 +581,7 @@ int32_t cwi_hash_blocks(cw_ctx* ctx, const i32* d_tokens, const u64* d_tok_off, 
     u64 max_units = (ctx->cfg.max_hashed_blocks >> CWH_UNIT_LOG2) + R;
     int grid = (int)((u64)ctx->hash_grid < max_units ? (u64)ctx->hash_grid : max_units);
     if (grid < 1) grid = 1;
-    hash_kernel<<<grid, CWH_UNIT + 32, sizeof(HashSmem), ctx->s_main>>>(a);
+    hash_kernel<<<grid, CWH_THREADS, sizeof(HashSmem), ctx->s_main>>>(a);
     CW_LAUNCH_CHECK(ctx);
     return CW_OK;
 }

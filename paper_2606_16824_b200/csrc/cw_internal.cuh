@@ -59,12 +59,14 @@ __host__ __device__ __forceinline__ u64 cw_remap_key(u64 k) {
 }
 
 // ---- stage 1 launch geometry ---------------------------------------------------------------------------
-#define CWH_WARPS 8                   // consumer warps per CTA
-#define CWH_UNIT (32 * CWH_WARPS)     // blocks per unit (one unit = one CTA iteration)
+#define CWH_WARPS 4                   // consumer warps per CTA; each takes a whole unit at a time
+#define CWH_K 8                       // consecutive blocks a consumer lane owns inside a unit
+#define CWH_UNIT (32 * CWH_K)         // blocks per unit (one unit = one TMA copy = one consumer-warp iteration)
 #define CWH_UNIT_LOG2 8
 #define CWH_SMALL_R 512                // calls with at most this many requests skip the plan kernel
-#define CWH_STAGES 3                  // smem ring depth
-#define CWH_MIN_CTAS 4
+#define CWH_STAGES 4                  // smem ring depth
+#define CWH_MIN_CTAS 3
+#define CWH_THREADS (32 * (CWH_WARPS + 1))
 #define CWH_STAGE_BYTES (CWH_UNIT * 64 + 16)
 
 struct cw_hash_rec {  // what the CTA of one range publishes for the CTA of the next range

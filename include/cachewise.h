@@ -114,6 +114,26 @@ int32_t cw_hash_blocks(cw_ctx* ctx, const int32_t* d_tokens, const uint64_t* d_t
                        const uint32_t* d_start_block, const uint64_t* d_start_state, const uint64_t* d_salt,
                        const uint64_t* d_hash_off, uint32_t R, uint64_t* d_hashes);
 
+/* cw_hash_blocks without a ctx and WITHOUT ANY ALLOCATION — for callers that cannot call cudaMalloc (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid it) and therefore cannot cw_create.  Same operation, same
+ * kernels and same argument meaning as cw_hash_blocks (stage 1, reading R1); the scratch a ctx would own
+ * (unit offsets, plan words, per-CTA hand-over records) is a fixed file-scope device array of about 164 KiB that every
+ * GPU loading the library holds until the process exits.  The call issues one 16-byte cudaMemsetAsync and one or two
+ * kernels on `stream`, on the CURRENT device; it calls no cudaMalloc / cudaFree / allocating routine.
+ *   R                  at most CW_HASH_STATIC_MAX_REQUESTS, else CW_E_INVAL (and a line on stderr); 0 = no-op
+ *   max_hashed_blocks  capacity of d_hashes in blocks: hash_off[R]-hash_off[0] beyond it is reported, nothing written
+ *   d_status           uint32 device word or NULL: device-detected conditions (the ones cw_hash_blocks reports at
+ *                      cw_sync) are OR-ed into it as a non-zero value; the caller clears and reads it
+ *   stream             cudaStream_t; NULL = legacy default stream
+ * All calls share the one scratch array: calls that OVERLAP on the GPU (two streams, two graph branches, two host
+ * threads) race — serialise them.  The array keeps the last call's contents; the call clears what must start at
+ * zero itself. */
+#define CW_HASH_STATIC_MAX_REQUESTS 16384u
+int32_t cw_hash_blocks_static(const int32_t* d_tokens, const uint64_t* d_tok_off, const uint32_t* d_start_block,
+                              const uint64_t* d_start_state, const uint64_t* d_salt, const uint64_t* d_hash_off,
+                              uint32_t R, uint64_t max_hashed_blocks, uint64_t* d_hashes, uint32_t* d_status,
+                              void* stream);
+
 /* Stage 2a — prefix overlap k_i(t) ("k_i(t) ... already reside in memory", L173 contiguous
  * prefix, Fig. 11B "overlap with KVCache resident on the XPU").  DESIGN.md reading R2.
  *   d_k_total uint32[R]: length of the LEADING run of resident hashes (either tier)

@@ -27,7 +27,7 @@ EXPORTS = ["cw_create", "cw_destroy", "cw_sync", "cw_join_copy", "cw_last_error"
            "cw_match_prefix", "cw_schedule", "cw_admit_chunked", "cw_score_evict", "cw_score_evict_begin", "cw_score_evict_end",
            "cw_predict_tau", "cw_swap_out", "cw_swap_in", "cw_gather_pages", "cw_scatter_pages", "cw_table_insert",
            "cw_table_erase", "cw_table_retag", "cw_table_lookup", "cw_table_compact", "cw_table_stats",
-           "cw_blocks_update"]
+           "cw_blocks_update", "cw_hash_blocks_static"]
 DEBUG_EXPORTS = ["cw_debug_evict_times", "cw_debug_stamp", "cw_debug_stamps"]  # libcachewise_debug.so only
 
 
@@ -74,6 +74,7 @@ def lib():
         L.cw_launch_count.argtypes = [P]
         L.cw_launch_count.restype = U64
         L.cw_hash_blocks.argtypes = [P, P, P, P, P, P, P, U32, P]
+        L.cw_hash_blocks_static.argtypes = [P, P, P, P, P, P, U32, U64, P, P, P]
         L.cw_match_prefix.argtypes = [P, P, P, U32, P, P, P]
         L.cw_schedule.argtypes = [P, U32, P, P, P, P, U32, U32, U32, U32, P, P, P]
         L.cw_admit_chunked.argtypes = [P, U32, P, P, P, P, U32, U32, U32, U64, P, P, P]
@@ -97,6 +98,20 @@ def lib():
                 getattr(L, name).restype = I32
         _lib = L
     return _lib
+
+
+HASH_STATIC_MAX_REQUESTS = 16384
+
+
+def hash_blocks_static(tokens, tok_off, hash_off, R, hashes, max_hashed_blocks, start_block=None, start_state=None,
+                       salt=None, status=None, stream=None):
+    """cw_hash_blocks_static: stage 1 with no ctx and no allocation (fixed static device scratch; at most
+    HASH_STATIC_MAX_REQUESTS requests per call; calls that overlap on the GPU race).  `stream` = raw cudaStream_t
+    (int) or None for the legacy default stream; asynchronous on it."""
+    rc = lib().cw_hash_blocks_static(_ptr(tokens), _ptr(tok_off), _ptr(start_block), _ptr(start_state), _ptr(salt),
+                                     _ptr(hash_off), R, max_hashed_blocks, _ptr(hashes), _ptr(status), stream)
+    if rc != CW_OK:
+        raise CwError(rc, "cw_hash_blocks_static")
 
 
 def _ptr(x):

@@ -33,7 +33,10 @@
 //                      then the boundary patch (about half a request per CTA: ~1% extra traffic, L2-resident)
 // Requests start at arbitrary 4-byte alignment: the copy starts at the 16-byte boundary below and the
 // consumers funnel the `mis` leading words away in registers.
+#include <stddef.h>
 #include <stdio.h>
+
+#include <mutex>
 
 #include "cw_internal.cuh"
 
@@ -585,3 +588,130 @@ int32_t cwi_hash_blocks(cw_ctx* ctx, const i32* d_tokens, const u64* d_tok_off, 
     CW_LAUNCH_CHECK(ctx);
     return CW_OK;
 }
+
+// ------------------------------------------------------------------------------------- no-allocation entry point
+// cw_hash_blocks_static: the same two kernels, for callers that can create no cw_ctx because they may not call
+// cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).  The scratch the ctx
+// would own — unit_off[R+1], the plan words, one hand-over record per CTA, a status word — lives in ONE file-scope
+// device array of fixed size (CWH_STATIC_BYTES, about 164 KiB), held by every GPU that loads the library until the
+// process exits.  Limits: R <= CW_HASH_STATIC_MAX_REQUESTS; any number of blocks.
+//
+// Host code must not hand `g_hash_static` itself to a kernel: in host code that name is a host-side stand-in, not a
+// device address.  The device address is fetched once per device with cudaGetSymbolAddress (that device current) and
+// kept in g_static_dev[]; the kernels get that pointer.
+//
+// Every call shares the array and it keeps the last call's contents.  What must start at zero — the range ticket and
+// the CTAs-done counter — is cleared at the start of every call (cudaMemsetAsync on the caller's stream: no
+// allocation); the epoch word deliberately persists (records of earlier calls go stale by epoch); unit_off and the
+// records are rewritten before they are read.  Two calls that overlap on the GPU (different streams, or graph branches)
+// RACE on the array: the caller serialises them.
+namespace {
+
+constexpr u32 CWH_STATIC_MAX_R = 16384;    // == CW_HASH_STATIC_MAX_REQUESTS in cachewise.h
+constexpr u32 CWH_STATIC_MAX_GRID = 2048;  // hand-over records (the grid is clamped to this)
+
+struct HashStaticScratch {
+    u64 unit_off[CWH_STATIC_MAX_R + 1];
+    u64 plan[4];  // [0] total units, [1] call epoch, [2] range ticket, [3] CTAs done
+    cw_hash_rec rec[CWH_STATIC_MAX_GRID];
+    u32 status;   // device-detected conditions when the caller passes no d_status
+    u32 pad[3];
+};
+constexpr size_t CWH_STATIC_BYTES = sizeof(HashStaticScratch);
+static_assert(CWH_STATIC_BYTES <= (192u << 10), "the static scratch is meant to stay modest");
+
+static __device__ __align__(256) unsigned char g_hash_static[CWH_STATIC_BYTES];
+
+struct StaticDev {
+    HashStaticScratch* scratch = nullptr;  // DEVICE address of g_hash_static on this device
+    int grid = 0;
+    bool ready = false;
+};
+constexpr int CWH_STATIC_MAX_DEVICES = 64;
+StaticDev g_static_dev[CWH_STATIC_MAX_DEVICES];
+std::mutex g_static_mu;
+
+// once per device, with that device current
+int32_t static_setup(int dev, StaticDev** out) {
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    StaticDev& d = g_static_dev[dev];
+    if (!d.ready) {
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_hash_static) != cudaSuccess || p == nullptr) return CW_E_CUDA;
+        int n_sm = 0;
+        if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n_sm < 1)
+            return CW_E_CUDA;
+        int grid = cwi_hash_grid(n_sm);  // sets the kernel's shared-memory opt-in on this device as well
+        if (cudaGetLastError() != cudaSuccess) return CW_E_CUDA;
+        d.scratch = static_cast<HashStaticScratch*>(p);
+        d.grid = grid < (int)CWH_STATIC_MAX_GRID ? grid : (int)CWH_STATIC_MAX_GRID;
+        d.ready = true;
+    }
+    *out = &d;
+    return CW_OK;
+}
+
+}  // namespace
+
+extern "C" {
+#pragma GCC visibility push(default)
+
+int32_t cw_hash_blocks_static(const int32_t* d_tokens, const uint64_t* d_tok_off, const uint32_t* d_start_block,
+                              const uint64_t* d_start_state, const uint64_t* d_salt, const uint64_t* d_hash_off,
+                              uint32_t R, uint64_t max_hashed_blocks, uint64_t* d_hashes, uint32_t* d_status,
+                              void* stream) {
+    if (R == 0) return CW_OK;
+    if (R > CWH_STATIC_MAX_R) {
+        fprintf(stderr, "cw_hash_blocks_static: R = %u exceeds the static scratch (at most %u requests per call)\n", R,
+                CWH_STATIC_MAX_R);
+        return CW_E_INVAL;
+    }
+    if (!d_tokens || !d_tok_off || !d_hash_off || !d_hashes) return CW_E_INVAL;
+    if (d_start_block && !d_start_state) return CW_E_INVAL;
+    if (!cw_aligned16(d_tokens) || (reinterpret_cast<uintptr_t>(d_tok_off) & 7) ||
+        (reinterpret_cast<uintptr_t>(d_hash_off) & 7) || (reinterpret_cast<uintptr_t>(d_hashes) & 7) ||
+        (reinterpret_cast<uintptr_t>(d_status) & 3))
+        return CW_E_INVAL;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return CW_E_CUDA;
+    if (dev < 0 || dev >= CWH_STATIC_MAX_DEVICES) return CW_E_INVAL;
+    StaticDev* sd = nullptr;
+    const int32_t rc = static_setup(dev, &sd);
+    if (rc != CW_OK) return rc;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    HashStaticScratch* sc = sd->scratch;  // device address; members are only ever dereferenced on the device
+
+    // what must start at zero: the range ticket and the CTAs-done counter (plan[2], plan[3]); the epoch stays
+    if (cudaMemsetAsync(reinterpret_cast<unsigned char*>(sc) + offsetof(HashStaticScratch, plan) + 2 * sizeof(u64), 0,
+                        2 * sizeof(u64), s) != cudaSuccess)
+        return CW_E_CUDA;
+    HashArgs a;
+    a.tokens = d_tokens;
+    a.tok_off = d_tok_off;
+    a.start_block = d_start_block;
+    a.start_state = d_start_state;
+    a.salt = d_salt;
+    a.hash_off = d_hash_off;
+    a.hashes = d_hashes;
+    a.unit_off = reinterpret_cast<u64*>(reinterpret_cast<unsigned char*>(sc) + offsetof(HashStaticScratch, unit_off));
+    a.plan = reinterpret_cast<u64*>(reinterpret_cast<unsigned char*>(sc) + offsetof(HashStaticScratch, plan));
+    a.rec = reinterpret_cast<cw_hash_rec*>(reinterpret_cast<unsigned char*>(sc) + offsetof(HashStaticScratch, rec));
+    a.status = d_status ? d_status
+                        : reinterpret_cast<u32*>(reinterpret_cast<unsigned char*>(sc) + offsetof(HashStaticScratch, status));
+    a.max_hashed = max_hashed_blocks;
+    a.R = R;
+    a.small = R <= CWH_SMALL_R ? 1u : 0u;
+    if (!a.small) {
+        hash_plan_kernel<<<1, 1024, 0, s>>>(a);
+        if (cudaGetLastError() != cudaSuccess) return CW_E_CUDA;
+    }
+    const u64 max_units = (max_hashed_blocks >> CWH_UNIT_LOG2) + R;
+    int grid = (int)((u64)sd->grid < max_units ? (u64)sd->grid : max_units);
+    if (grid < 1) grid = 1;
+    hash_kernel<<<grid, CWH_THREADS, sizeof(HashSmem), s>>>(a);
+    if (cudaGetLastError() != cudaSuccess) return CW_E_CUDA;
+    return CW_OK;
+}
+
+#pragma GCC visibility pop
+}  // extern "C"

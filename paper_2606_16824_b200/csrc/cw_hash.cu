@@ -105,14 +105,12 @@ __device__ __forceinline__ u64 pow_u64(u64 base, u64 e) {
 }
 
 // ------------------------------------------------------------------------------------------------ plan
-// Loads first, decisions after: a load behind a condition is not issued until the condition is known, and the plan
-// wants all of a thread's loads in flight at once.
 __device__ __forceinline__ u64 plan_units(const HashArgs& a, u32 r, bool too_big) {
+    if (too_big) return 0;
     const u64 t0 = a.tok_off[r], t1 = a.tok_off[r + 1], h0 = a.hash_off[r], h1 = a.hash_off[r + 1];
     const u64 sb = a.start_block ? a.start_block[r] : 0;
-    const bool invalid = t1 < t0 || h1 < h0 || (h1 - h0) != ((t1 - t0) >> 4) || sb > h1 - h0;
-    const u64 T = (h1 - h0 - sb + CWH_UNIT - 1) >> CWH_UNIT_LOG2;
-    return too_big ? 0ull : (invalid ? ~0ull : T);
+    if (t1 < t0 || h1 < h0 || (h1 - h0) != ((t1 - t0) >> 4) || sb > h1 - h0) return ~0ull;  // invalid request
+    return (h1 - h0 - sb + CWH_UNIT - 1) >> CWH_UNIT_LOG2;
 }
 
 __global__ void __launch_bounds__(1024) hash_plan_kernel(const HashArgs a) {
@@ -125,16 +123,10 @@ __global__ void __launch_bounds__(1024) hash_plan_kernel(const HashArgs a) {
     const u32 lo = min(R, tid * per), hi = min(R, lo + per);
     u64 local = 0;
     bool bad = false;
-    for (u32 r0 = lo; r0 < hi; r0 += 4) {  // four requests' loads in flight at once (clamped index, select after)
-        u64 T[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) T[k] = plan_units(a, min(r0 + k, hi - 1), too_big);
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const bool in = r0 + k < hi;
-            bad |= in && T[k] == ~0ull;
-            local += (in && T[k] != ~0ull) ? T[k] : 0ull;
-        }
+    for (u32 r = lo; r < hi; ++r) {
+        const u64 T = plan_units(a, r, too_big);
+        if (T == ~0ull) bad = true;
+        else local += T;
     }
     if (bad) atomicOr(a.status, CWS_INVAL);
     u64 inc = local;
@@ -163,17 +155,10 @@ __global__ void __launch_bounds__(1024) hash_plan_kernel(const HashArgs a) {
     }
     __syncthreads();
     u64 run = s_warp[warp] + inc - local;
-    for (u32 r0 = lo; r0 < hi; r0 += 4) {
-        u64 T[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) T[k] = plan_units(a, min(r0 + k, hi - 1), too_big);
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            if (r0 + k < hi) {
-                a.unit_off[r0 + k] = run;
-                if (T[k] != ~0ull) run += T[k];
-            }
-        }
+    for (u32 r = lo; r < hi; ++r) {
+        a.unit_off[r] = run;
+        const u64 T = plan_units(a, r, too_big);
+        if (T != ~0ull) run += T;
     }
 }
 

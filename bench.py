@@ -42,25 +42,52 @@ STAGE_KERNEL = {"hash": "hash_kernel", "match": "match_probe_kernel", "schedule"
                 "score_evict": "evict_kernel", "gather": "copy_pages_kernel<true>", "scatter": "copy_pages_kernel<false>"}
 
 
-def ncu_traffic():
-    """{stage: bytes per launch} from the committed raw ncu export (the LAST launch of each kernel), or {}."""
+def _ncu_rows():
+    """(head, units, rows) of the committed raw ncu export, kernel names normalised; None if absent."""
     import csv
     if not os.path.exists(NCU_RAW):
-        return {}
+        return None
+    rows = list(csv.reader(open(NCU_RAW)))
+    head, units = rows[0], rows[1]
+    ki = head.index("Kernel Name")
+    body = []
+    for r in rows[2:]:
+        if len(r) == len(head):
+            r = list(r)
+            r[ki] = (r[ki].replace("(bool)1", "true").replace("(bool)0", "false")
+                     .replace("kernel<1>", "kernel<true>").replace("kernel<0>", "kernel<false>"))
+            body.append(r)
+    return head, units, body
+
+
+def ncu_traffic():
+    """{stage: bytes per launch} from the committed raw ncu export (the LAST launch of each kernel), or {}."""
     try:
-        rows = list(csv.reader(open(NCU_RAW)))
-        head, units = rows[0], rows[1]
+        head, units, rows = _ncu_rows()
         ki, ri, wi = head.index("Kernel Name"), head.index("dram__bytes_read.sum"), head.index("dram__bytes_write.sum")
         scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
         out = {}
-        for r in rows[2:]:
-            if len(r) <= max(ki, ri, wi):
-                continue
+        for r in rows:
             for stage, kern in STAGE_KERNEL.items():
-                name = (r[ki].replace("(bool)1", "true").replace("(bool)0", "false")
-                        .replace("kernel<1>", "kernel<true>").replace("kernel<0>", "kernel<false>"))
-                if kern in name:
+                if kern in r[ki]:
                     out[stage] = int(float(r[ri]) * scale.get(units[ri], 1.0) + float(r[wi]) * scale.get(units[wi], 1.0))
+        return out
+    except Exception:
+        return {}
+
+
+def ncu_kernel_us():
+    """{stage: device time (us) of the stage's main kernel ALONE} from the same committed capture (cold cache,
+    serialised by ncu): context beside the live stage times, which are whole calls (e.g. plan kernel + hash kernel)."""
+    try:
+        head, units, rows = _ncu_rows()
+        ki, ti = head.index("Kernel Name"), head.index("gpu__time_duration.sum")
+        scale = {"ns": 1e-3, "us": 1.0, "ms": 1e3, "s": 1e6}
+        out = {}
+        for r in rows:
+            for stage, kern in STAGE_KERNEL.items():
+                if kern in r[ki]:
+                    out[stage] = round(float(r[ti]) * scale.get(units[ti], 1.0), 2)
         return out
     except Exception:
         return {}
@@ -462,6 +489,7 @@ def run_cuda(args):
     decide_ms = per3[0]
     alg = st.algorithmic_bytes(nv)
     traffic = ncu_traffic()
+    kern_us = ncu_kernel_us() if args.scale <= 1 else {}
     rooflines = {}
     for name in st.STAGES:
         if name in stage_ms and stage_ms[name] > 0:
@@ -469,6 +497,9 @@ def run_cuda(args):
             rooflines[name] = {"bound": "hbm", "achieved": round(ach, 1), "peak": hbm_peak, "unit": "GB/s",
                                "frac": round(ach / hbm_peak, 4), "traffic": traffic.get(name) if args.scale <= 1 else None,
                                "algorithmic_bytes": alg[name], "us": round(stage_ms[name] * 1e3, 2)}
+            if name in kern_us and name != "score_evict":   # the captured evict launch is the 37-CTA speculative one
+                rooflines[name]["main_kernel_alone_us_ncu"] = kern_us[name]
+                rooflines[name]["main_kernel_alone_frac_ncu"] = round(alg[name] / kern_us[name] / 1e3 / hbm_peak, 4)
     dominant = max(stage_ms, key=stage_ms.get)
     roofline = dict(rooflines[dominant], kernel=dominant, peak_source=peak_src,
                     traffic_source="profiles/r2_step_kernels_raw.csv" if traffic else None,

@@ -179,3 +179,5 @@ def test_bench_reads_roofline_traffic_from_the_committed_ncu_export():
     assert 0.85 * 421e6 < t["hash"] < 1.15 * 475e6                              # the token ids, once
     md = open(os.path.join(ROOT, "profiles", "r2_step_kernels_raw.md")).read()
     assert "ncu --set full" in md and "bench.py" in md                            # the export names its command
+    us = bench.ncu_kernel_us()                                                    # the main kernel of each stage alone
+    assert set(us) == set(t) and 64 < us["hash"] < 130 and 200 < us["gather"] < 320

@@ -165,12 +165,12 @@ class StressStep:
         """Stages 1-3 (the <=100 us target of BASELINE.json).  overlap: the selection of the eviction budget runs on
         the ctx's side stream beside hash -> match -> schedule (cw_score_evict_begin / _end); otherwise the four
         calls run in series."""
-        # a cold step hashes 421 MB of token ids and wants every SM for it: the fork comes after the hash there
-        if overlap and steady:
+        # the fork comes first in both kinds of step: the round-2 hash kernel (4 + 1 warps, 3 CTAs per SM) no longer
+        # loses more to the selection's 37 SMs than the match gains from the earlier start (cold: 211-215 us against
+        # 215-221 us with the fork after the hash; with the round-1 hash kernel it was the other way round)
+        if overlap:
             self.score_evict_begin()
         self.hash(steady)
-        if overlap and not steady:
-            self.score_evict_begin()
         self.match()
         self.schedule()
         if overlap:

@@ -21,12 +21,9 @@ def main():
         st.decide(False); st.decide(True); stream.synchronize()
         for name, steady in (("steady", True), ("cold", False)):
             for rep in range(3):
-                if steady:
-                    fns = [st.score_evict_begin, lambda: st.hash(True), st.match, st.schedule, st.score_evict_end]
-                    labels = ["begin (fork)", "hash (256 new requests)", "match", "schedule", "end (join + trim)"]
-                else:
-                    fns = [lambda: st.hash(False), st.score_evict_begin, st.match, st.schedule, st.score_evict_end]
-                    labels = ["hash (all 4096 requests)", "begin (fork)", "match", "schedule", "end (join + trim)"]
+                fns = [st.score_evict_begin, lambda: st.hash(steady), st.match, st.schedule, st.score_evict_end]
+                labels = ["begin (fork)", "hash (256 new requests)" if steady else "hash (all 4096 requests)", "match",
+                          "schedule", "end (join + trim)"]
                 main, ev = st.ctx.debug_timeline(fns)
             t0 = main[0]
             print(f"== {name} step, us from the first stamp on stream_main")

@@ -646,6 +646,12 @@ def run_cuda(args):
             for name, steady in (("cold", False), ("steady", True)):
                 dec[name + "_l2_warm"] = graph_latency(torch, stream, lambda: st.decide(steady))
                 dec[name + "_l2_flushed"] = graph_latency(torch, stream, lambda: st.decide(steady), flush=flush)
+            # stage 2a alone as a one-call graph: the step's call (shared prefixes looked up once) and the plain call
+            dec["match_shared_l2_flushed"] = graph_latency(torch, stream, st.match, flush=flush)
+            st.shared_match = False
+            dec["match_plain_l2_flushed"] = graph_latency(torch, stream, st.match, flush=flush)
+            dec["steady_plain_match_l2_flushed"] = graph_latency(torch, stream, lambda: st.decide(True), flush=flush)
+            st.shared_match = True
         del big
         with torch.cuda.stream(stream):  # the steady-state hash call alone (CUDA events, median of 20)
             ts = []
@@ -659,7 +665,9 @@ def run_cuda(args):
             dec["steady_hash_us"] = round(sorted(ts[3:])[10], 2)
         dec["note"] = ("stages 1-3 (hash, match, schedule, score/select) as one CUDA graph; cold = all 4096 requests "
                        f"hashed ({st.n_hashed} blocks), steady = hashes persist and the {st.new_requests} newest "
-                       f"requests ({st.n_hashed_new} blocks) are hashed; target <= 100 us")
+                       f"requests ({st.n_hashed_new} blocks) are hashed; target <= 100 us; stage 2a = "
+                       "cw_match_prefix_shared with the longest queued request of a session as the leader hint "
+                       "(steady_plain_match = the same step through cw_match_prefix)")
         extra["decision_step"] = dec
 
     st.close()
@@ -737,6 +745,7 @@ def run_cuda(args):
                        "tokens_per_step": int(snap.tok_off[-1]), "victims_per_step": nv,
                        "kv_page_bytes": stress.STEP_N_CHUNKS * stress.STEP_CHUNK_BYTES,
                        "l2": "inputs larger than L2 (token ids + swap traffic per step >> 126 MB); no flush",
+                       "match": "cw_match_prefix_shared, leader hint = longest queued request of the session",
                        "parallelism": f"replicas x{world} (no collective)", "status": status, "scale": args.scale},
             "roofline": roofline, "rooflines": rooflines,
             "stages_us": dict({k: round(v * 1e3, 2) for k, v in stage_ms.items()},

@@ -32,6 +32,17 @@ def host(t, dtype):
     return t.cpu().numpy().view(dtype)
 
 
+def session_leaders(req_session, hash_off):
+    """The hint cw_match_prefix_shared takes: for every queued request the index of the LONGEST queued request of its
+    session (what a scheduler that keeps its queue per session knows; none of the method's arithmetic)."""
+    n = (hash_off[1:] - hash_off[:-1]).astype(np.int64)
+    order = np.lexsort((np.arange(n.size), -n, req_session))      # per session: longest first, lowest index on ties
+    first = np.ones(n.size, bool)
+    first[1:] = req_session[order][1:] != req_session[order][:-1]
+    lead_of_session = {int(s): int(i) for s, i in zip(req_session[order][first], order[first])}
+    return np.array([lead_of_session[int(s)] for s in req_session], np.uint32)
+
+
 def hash_off_of(tok_off):
     tok_off = np.asarray(tok_off, np.uint64)
     n = (tok_off[1:] - tok_off[:-1]) // np.uint64(16)
@@ -54,7 +65,8 @@ class StressStep:
     def __init__(self, snap: gen.StressSnapshot, stream: torch.cuda.Stream, with_pool: bool = True,
                  layout: str = "block", n_chunks: int = STEP_N_CHUNKS, chunk_bytes: int = STEP_CHUNK_BYTES,
                  staging_bytes: int = 128 << 20, policy: int = cw.POLICY_MIN_ADDITIONAL, free_blocks: int = 0,
-                 holes: bool = False, new_requests: int = 256, spec_ctas: int = 0, stream_copy=None):
+                 holes: bool = False, new_requests: int = 256, spec_ctas: int = 0, stream_copy=None,
+                 shared_match: bool = True):
         self.snap, self.stream = snap, stream
         S, L = snap.streams.shape
         self.S, self.L, self.RB, self.M = S, L, snap.resident_blocks, snap.M
@@ -62,6 +74,7 @@ class StressStep:
         self.F = snap.features.shape[1]
         self.policy, self.free_blocks = policy, free_blocks
         self.spec_ctas = spec_ctas                # CTAs of the speculative selection (0 = library default)
+        self.shared_match = shared_match          # stage 2a through cw_match_prefix_shared (leader = longest of the session)
         self.evict_budget = snap.deficit          # "eviction deficit 5% of the pool per step"
         self.cap = max(snap.deficit, 1)
         self.page = n_chunks * chunk_bytes
@@ -107,6 +120,7 @@ class StressStep:
             self.d_tok = dev(np.concatenate([snap.tokens, np.zeros(4, np.int32)]))
             self.d_tok_off, self.d_hash_off = dev(snap.tok_off), dev(self.hash_off)
             self.d_need, self.d_arr, self.d_rid = dev(snap.need_d), dev(snap.arrival_seq), dev(snap.req_id)
+            self.d_leader = dev(session_leaders(snap.req_session, self.hash_off))
             self.d_feat, self.d_w = dev(snap.features), dev(snap.weights)
             self.d_state = dev(snap.session_state)
             R = self.R
@@ -136,7 +150,11 @@ class StressStep:
             self.ctx.hash_blocks(self.d_tok, self.d_tok_off, self.d_hash_off, self.R, self.d_hashes)
 
     def match(self):
-        self.ctx.match_prefix(self.d_hashes, self.d_hash_off, self.R, self.d_k, self.d_g, self.d_loc)
+        if self.shared_match:
+            self.ctx.match_prefix_shared(self.d_hashes, self.d_hash_off, self.R, self.d_leader, self.d_k, self.d_g,
+                                         self.d_loc)
+        else:
+            self.ctx.match_prefix(self.d_hashes, self.d_hash_off, self.R, self.d_k, self.d_g, self.d_loc)
 
     def schedule(self):
         self.ctx.schedule(self.R, self.d_need, self.d_g, self.d_arr, self.d_rid, self.policy, self.free_blocks,

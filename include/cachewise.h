@@ -144,6 +144,21 @@ int32_t cw_hash_blocks_static(const int32_t* d_tokens, const uint64_t* d_tok_off
 int32_t cw_match_prefix(cw_ctx* ctx, const uint64_t* d_hashes, const uint64_t* d_hash_off, uint32_t R,
                         uint32_t* d_k_total, uint32_t* d_n_gpu, uint32_t* d_hit_loc);
 
+/* cw_match_prefix for a queue whose requests SHARE PREFIXES (an agent workload queues many requests of one session:
+ * PAPER.md L173 "contiguous prefix", Fig. 11B; configs[2] repeats 5.4 M of its 6.6 M lookups).  Same outputs
+ * as cw_match_prefix, bit for bit, under the precondition below; the shared part of a request is looked up once.
+ *   d_leader uint32[R]: for request r the index of a request of the same call that is expected to start with the same
+ *            hashes (e.g. the longest queued request of r's session; the scheduler knows the session of a request);
+ *            d_leader[r] = r for a request that probes on its own.  A hint is only a hint: an index >= R, a
+ *            leader that is not its own leader, or a leader that shares nothing costs one search and the request is
+ *            probed on its own.
+ * PRECONDITION: d_hashes are CHAIN hashes as cw_hash_blocks writes them (the hash of block p is a function of the
+ * whole token prefix), so two requests whose hashes agree at position p agree at every position before p.  The
+ * length of the shared prefix is found by a search that relies on it; hashes without that property give unspecified
+ * (but memory-safe) results — use cw_match_prefix for those. */
+int32_t cw_match_prefix_shared(cw_ctx* ctx, const uint64_t* d_hashes, const uint64_t* d_hash_off, uint32_t R,
+                               const uint32_t* d_leader, uint32_t* d_k_total, uint32_t* d_n_gpu, uint32_t* d_hit_loc);
+
 /* Stage 2b — prefix-aware scheduling (PAPER.md 5.1 L207 "fewest additional blocks a_i(t)", L177 a_i = d_i-k_i
  * and admission W+a_i <= M, L281 FCFS baseline).  DESIGN.md reading R3.
  *   d_need uint32[R] = d_r = ceil(len_r/16);  a_r = max(d_r - n_gpu_r, 0)

@@ -27,7 +27,7 @@ EXPORTS = ["cw_create", "cw_destroy", "cw_sync", "cw_join_copy", "cw_last_error"
            "cw_match_prefix", "cw_schedule", "cw_admit_chunked", "cw_score_evict", "cw_score_evict_begin", "cw_score_evict_end",
            "cw_predict_tau", "cw_swap_out", "cw_swap_in", "cw_gather_pages", "cw_scatter_pages", "cw_table_insert",
            "cw_table_erase", "cw_table_retag", "cw_table_lookup", "cw_table_compact", "cw_table_stats",
-           "cw_blocks_update", "cw_hash_blocks_static"]
+           "cw_blocks_update", "cw_hash_blocks_static", "cw_match_prefix_shared"]
 DEBUG_EXPORTS = ["cw_debug_evict_times", "cw_debug_stamp", "cw_debug_stamps"]  # libcachewise_debug.so only
 
 
@@ -76,6 +76,7 @@ def lib():
         L.cw_hash_blocks.argtypes = [P, P, P, P, P, P, P, U32, P]
         L.cw_hash_blocks_static.argtypes = [P, P, P, P, P, P, U32, U64, P, P, P]
         L.cw_match_prefix.argtypes = [P, P, P, U32, P, P, P]
+        L.cw_match_prefix_shared.argtypes = [P, P, P, U32, P, P, P, P]
         L.cw_schedule.argtypes = [P, U32, P, P, P, P, U32, U32, U32, U32, P, P, P]
         L.cw_admit_chunked.argtypes = [P, U32, P, P, P, P, U32, U32, U32, U64, P, P, P]
         L.cw_score_evict.argtypes = [P, U32, U32, U32, P, P, I32, P, P, P, U32, P, P, P, U32]
@@ -207,6 +208,10 @@ class Context:
     def match_prefix(self, hashes, hash_off, R, k_total, n_gpu, hit_loc=None):
         self._ck(lib().cw_match_prefix(self._h, _ptr(hashes), _ptr(hash_off), R, _ptr(k_total), _ptr(n_gpu),
                                        _ptr(hit_loc)), "cw_match_prefix")
+
+    def match_prefix_shared(self, hashes, hash_off, R, leader, k_total, n_gpu, hit_loc=None):
+        self._ck(lib().cw_match_prefix_shared(self._h, _ptr(hashes), _ptr(hash_off), R, _ptr(leader), _ptr(k_total),
+                                              _ptr(n_gpu), _ptr(hit_loc)), "cw_match_prefix_shared")
 
     def schedule(self, R, need, n_gpu, arrival_seq, req_id, policy, free_blocks, evictable, max_admit, order,
                  num_admit, deficit):

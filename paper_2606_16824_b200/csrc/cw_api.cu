@@ -50,6 +50,8 @@ void free_all(cw_ctx* c) {
     cudaFree(c->m_first_miss);
     cudaFree(c->m_max_hit);
     cudaFree(c->m_host_hits);
+    cudaFree(c->m_shared);
+    cudaFree(c->m_list);
     cudaFree(c->sched_a);
     cudaFree(c->tau_q);
     cudaFree(c->out_score);
@@ -134,6 +136,8 @@ int32_t cw_create(const cw_config* cfg, cw_ctx** out) {
     CW_CUDA(c, dalloc_zero(&c->m_first_miss, cfg->max_requests, s, 0xFF));
     CW_CUDA(c, dalloc_zero(&c->m_max_hit, cfg->max_requests, s));
     CW_CUDA(c, dalloc_zero(&c->m_host_hits, cfg->max_requests, s));
+    CW_CUDA(c, dalloc_zero(&c->m_shared, 4 * (size_t)cfg->max_requests + 1, s));
+    CW_CUDA(c, dalloc_zero(&c->m_list, 2 * ((size_t)(cfg->max_hashed_blocks / 128) + cfg->max_requests + 2), s));
     // stage 2b
     CW_CUDA(c, dalloc_zero(&c->sched_a, cfg->max_requests, s));
     // stage 3
@@ -269,6 +273,14 @@ int32_t cw_match_prefix(cw_ctx* ctx, const uint64_t* d_hashes, const uint64_t* d
     if (R == 0) return CW_OK;
     if (!d_hashes || !d_hash_off || !d_k_total || !d_n_gpu || R > ctx->cfg.max_requests) return CW_E_INVAL;
     return cwi_match_prefix(ctx, d_hashes, d_hash_off, R, d_k_total, d_n_gpu, d_hit_loc);
+}
+
+int32_t cw_match_prefix_shared(cw_ctx* ctx, const uint64_t* d_hashes, const uint64_t* d_hash_off, uint32_t R,
+                               const uint32_t* d_leader, uint32_t* d_k_total, uint32_t* d_n_gpu, uint32_t* d_hit_loc) {
+    if (!ctx) return CW_E_STATE;
+    if (R == 0) return CW_OK;
+    if (!d_hashes || !d_hash_off || !d_leader || !d_k_total || !d_n_gpu || R > ctx->cfg.max_requests) return CW_E_INVAL;
+    return cwi_match_prefix_shared(ctx, d_hashes, d_hash_off, R, d_leader, d_k_total, d_n_gpu, d_hit_loc);
 }
 
 int32_t cw_schedule(cw_ctx* ctx, uint32_t R, const uint32_t* d_need, const uint32_t* d_n_gpu,

@@ -141,6 +141,8 @@ struct cw_ctx {
     u32* m_first_miss;
     u32* m_max_hit;
     u32* m_host_hits;
+    u32* m_shared;  // cw_match_prefix_shared: first_miss, max_hit, host_hits, lcp [max_requests each], list length [1]
+    u32* m_list;  // cw_match_prefix_shared: (task, request) pairs of the 128-position tasks that hold something to probe
     // stage 2b
     u32* sched_a;       // a of every request in dispatch order (max_requests)
     // stage 3
@@ -285,6 +287,7 @@ __device__ __forceinline__ u64 ld_relaxed_u64(const u64* p) {
 // per-TU entry points (host side), called from cw_api.cu
 int32_t cwi_hash_blocks(cw_ctx*, const i32*, const u64*, const u32*, const u64*, const u64*, const u64*, u32, u64*);
 int32_t cwi_match_prefix(cw_ctx*, const u64*, const u64*, u32, u32*, u32*, u32*);
+int32_t cwi_match_prefix_shared(cw_ctx*, const u64*, const u64*, u32, const u32*, u32*, u32*, u32*);
 int32_t cwi_table_insert(cw_ctx*, const u64*, const u32*, u32, u32*);
 int32_t cwi_table_erase(cw_ctx*, const u64*, u32);
 int32_t cwi_table_retag(cw_ctx*, const u64*, const u32*, u32);

@@ -314,7 +314,13 @@ __global__ void insert_reset_kernel(cw_slot* table, u32 n, const u32* ins_slot) 
 __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_kernel(const cw_slot* __restrict__ table, u32 mask,
                                                           const u64* __restrict__ hashes,
                                                           const u64* __restrict__ hash_off, u32 R, u32* first_miss,
-                                                          u32* max_hit, u32* host_hits, u32* hit_loc, u32* status) {
+                                                          u32* max_hit, u32* host_hits, u32* hit_loc, u32* status,
+                                                          const u32* __restrict__ lcp, const uint2* __restrict__ list,
+                                                          const u32* __restrict__ list_n) {
+    // lcp (cw_match_prefix_shared only, else NULL): request r is probed from position lcp[r] on (~0: from 0); the
+    // positions in front of it are answered from its leader's results by match_share_kernel; list[0 .. *list_n) are
+    // the tasks that hold at least one position to probe (in no particular order), each with the request its first
+    // position lies in (what the search below would find)
     __shared__ u64 s_key[MATCH_THREADS / 32][CWM_CHUNK];
     __shared__ u32 s_loc[MATCH_THREADS / 32][CWM_CHUNK];
     // hash_off may be a slice of a longer CSR array: positions below are 32-bit offsets from its first hash
@@ -328,14 +334,16 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
     u32* hl = hit_loc ? hit_loc + h_first : nullptr;
     const u32 lane = threadIdx.x & 31;
     const u32 nwarps = (gridDim.x * blockDim.x) >> 5;
-    const u32 n_tasks = (total + CWM_CHUNK - 1) / CWM_CHUNK;
+    const u32 n_tasks = list ? *list_n : (total + CWM_CHUNK - 1) / CWM_CHUNK;
     // a warp walks its task front to back, so once it has seen a miss of a request the rest of that request is
     // answered without touching the table (the leading run is over); a miss recorded by an earlier task of the
     // same request is honoured too when the warp enters that request
-    for (u32 w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; w < n_tasks; w += nwarps) {
-        const u32 c0 = w * CWM_CHUNK;
+    for (u32 wi = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; wi < n_tasks; wi += nwarps) {
+        uint2 le = make_uint2(wi, 0u);
+        if (list) le = list[wi];
+        const u32 c0 = le.x * CWM_CHUNK;
         // largest r with hash_off[r] <= c0 (r < R), 32-ary search, warp-uniform, once per task
-        u32 lo = 0, hi = R;
+        u32 lo = le.y, hi = list ? lo + 1 : R;
         while (hi - lo > 1) {
             u32 step = (hi - lo + 31) >> 5;
             u32 p = lo + lane * step;
@@ -355,6 +363,14 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
             // iteration of a warp-synchronous loop, so the warp waits for the longest SUM of probe lengths over a
             // lane's keys instead of the sum over rounds of the longest probe of the round.
             const u32 j0 = c0 - req_start;
+            u32 skip = 0;  // leading positions of the task that belong to the shared prefix (not probed here)
+            if (lcp) {
+                const u32 from = lcp[r_base];
+                if (from != 0xFFFFFFFFu) {
+                    if (from >= j0 + (c1 - c0)) continue;  // the whole task is answered from the leader
+                    skip = from > j0 ? from - j0 : 0u;
+                }
+            }
             if (j0 > 0 && __ldcg(first_miss + r_base) < j0) {  // an earlier task of the request already missed
                 if (hl)
                     for (u32 g = c0 + lane; g < c1; g += 32) __stcs(hl + g, CW_MISS);
@@ -375,8 +391,9 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
                 for (int q = 0; q < KPL; ++q) wkey[lane + 32 * q] = cw_remap_key(kk[q]);  // read back by this lane only
             }
             u32 pos = lane;          // position of this lane's current key inside the task
+            if (skip > lane) pos += (skip - lane + 31) & ~31u;  // first position of this lane at or behind `skip`
             u32 limit = n_task;      // warp-uniform: min(n_task, first missing position seen so far)
-            uint2 key = *reinterpret_cast<const uint2*>(wkey + pos);
+            uint2 key = *reinterpret_cast<const uint2*>(wkey + (pos & (CWM_CHUNK - 1)));
             const u32 pmask = mask >> 1;          // the table as pairs of slots: one 32-byte sector each
             u32 pair = (key.x & mask) >> 1;       // homes are even slots
             for (;;) {
@@ -414,14 +431,14 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
 #pragma unroll
             for (int q = 0; q < KPL; ++q) {
                 const u32 p = lane + 32 * q;
-                const u32 l = p < limit ? wloc[p] : CW_MISS;
+                const u32 l = (p < limit && p >= skip) ? wloc[p] : CW_MISS;
                 host += (l != CW_MISS && (l & CW_HOST_BIT)) ? 1u : 0u;
-                if (hl && p < n_task) __stcs(hl + c0 + p, l);  // streaming: hit_loc is not re-read on the device
+                if (hl && p < n_task && p >= skip) __stcs(hl + c0 + p, l);  // streaming: not re-read by this kernel
             }
             host = __reduce_add_sync(0xffffffffu, host);
             if (lane == 0) {
                 if (limit < n_task) atomicMin(&first_miss[r_base], j0 + limit);
-                if (limit) atomicMax(&max_hit[r_base], j0 + limit);
+                if (limit > skip) atomicMax(&max_hit[r_base], j0 + limit);
                 if (host) atomicAdd(&host_hits[r_base], host);
             }
             __syncwarp();  // the staging rows are reused by the next task of this warp
@@ -435,7 +452,7 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
                 req_end = (u32)(hash_off[r_base + 1] - h_first);
             }
             const u32 g = g0 + lane;
-            const bool active = g < c1;
+            bool active = g < c1;
             const u64 key = key_next;
             if (g + 32 < c1) key_next = hs[g + 32];  // prefetch the next round
             u32 r = r_base;
@@ -446,6 +463,10 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
                     while (g >= (u32)(hash_off[r + 1] - h_first)) ++r;
                 j = active ? g - (u32)(hash_off[r] - h_first) : 0;
                 uniform = __all_sync(0xffffffffu, !active || r == r_base);
+            }
+            if (lcp && active) {  // positions of the shared prefix are not probed here
+                const u32 from = lcp[r];
+                if (from != 0xFFFFFFFFu && j < from) active = false;
             }
             if (uniform) {
                 if (r_base != checked_r && r_base != dead_r) {  // entering a request: did an earlier task miss?
@@ -520,6 +541,143 @@ __global__ void __launch_bounds__(256) match_finish_kernel(const u64* __restrict
         max_hit[r] = 0;
         host_hits[r] = 0;
     }
+}
+
+// ---------------------------------------------------------------------------------- match with shared prefixes
+// cw_match_prefix_shared.  The queue of an agent workload holds many requests of one session, and they repeat the
+// session's first thousands of hashes (configs[2]: 5.4 M of 6.6 M lookups).  The caller names, per request, a LEADER
+// (say the longest queued request of the session).  Because the hashes are CHAIN hashes (stage 1: H_j is a function of
+// the whole token prefix), two requests that agree at position p agree at every position before p, so
+//   match_lcp_kernel    finds L_r = number of leading hashes request r shares with its leader by a 32-ary search
+//                       (three rounds for 8192 blocks) without touching the table, and appends the 128-position
+//                       tasks that still hold something to probe to a compact list,
+//   match_probe_kernel  walks that list: leaders in full, every other request from position L_r on (its own tail),
+//   match_share_kernel  (one CTA per request) answers positions [0, L_r) of a follower from the leader's results,
+//                       computes k_total / n_gpu and resets the list counter.
+// A hint that shares nothing (or is not itself a leader) only costs the search: the request is probed on its own.
+#define SHARE_THREADS 128
+#define SHARE_UNROLL 8  // loads in flight per thread: a follower of 8192 shared blocks is copied in 8 rounds
+
+// one warp per request
+__global__ void __launch_bounds__(256) match_lcp_kernel(const u64* __restrict__ hashes, const u64* __restrict__ hash_off,
+                                                        u32 R, const u32* __restrict__ leader, u32* lcp, uint2* list,
+                                                        u32* list_n, u32* first_miss, u32* max_hit, u32* host_hits) {
+    const u32 lane = threadIdx.x & 31;
+    const u32 r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (r >= R) return;
+    const u64 h_first = hash_off[0];
+    if (hash_off[R] - h_first > 0xFFFFFFFFull) return;  // the probe kernel rejects the call: scratch stays armed
+    const u64 a0 = hash_off[r], a1 = hash_off[r + 1];
+    const u32 l = leader[r];
+    u32 out = 0xFFFFFFFFu;
+    if (l < R && l != r && leader[l] == l) {
+        const u64 b0 = hash_off[l];
+        const u64 n = min(a1 - a0, hash_off[l + 1] - b0);
+        const u64* __restrict__ ha = hashes + a0;
+        const u64* __restrict__ hb = hashes + b0;
+        u64 lo = 0, hi = n;  // every position below lo agrees; position hi (if < n) differs
+        while (lo < hi) {
+            const u64 step = (hi - lo + 31) >> 5;
+            const u64 p = lo + lane * step;
+            const bool tested = p < hi;
+            const bool differs = tested && ha[p] != hb[p];
+            const u32 dmask = __ballot_sync(0xffffffffu, differs);
+            const u32 tmask = __ballot_sync(0xffffffffu, tested);
+            if (dmask) {
+                const u32 first = (u32)__ffs(dmask) - 1;  // positions up to lane first-1 agree, lane first differs
+                hi = lo + first * step;
+                if (first) lo = lo + (first - 1) * step + 1;
+            } else {
+                lo = min(hi, lo + (u64)(32 - __clz(tmask) - 1) * step + 1);  // the last tested position agrees
+            }
+        }
+        if (lo > 0 && lo <= 0xFFFFFFFEull) out = (u32)lo;
+    }
+    if (lane == 0) {
+        lcp[r] = out;
+        // this path has its own per-request scratch and arms it here, in front of the probe kernel (the plain call's
+        // scratch is re-armed by its finish kernel; a grid-wide "last CTA re-arms" costs one contended atomic per CTA)
+        first_miss[r] = 0xFFFFFFFFu;
+        max_hit[r] = 0;
+        host_hits[r] = 0;
+    }
+    // the tasks whose FIRST position lies in this request, minus those that end inside the shared prefix
+    const u32 start = (u32)(a0 - h_first), end = (u32)(a1 - h_first);
+    const u32 t_hi = (end + CWM_CHUNK - 1) / CWM_CHUNK;
+    u32 t_lo = (start + CWM_CHUNK - 1) / CWM_CHUNK;
+    if (out != 0xFFFFFFFFu) t_lo = max(t_lo, (start + out) / CWM_CHUNK);
+    if (t_hi > t_lo) {
+        u32 base = 0;
+        if (lane == 0) base = atomicAdd(list_n, t_hi - t_lo);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        for (u32 i = lane; i < t_hi - t_lo; i += 32) list[base + i] = make_uint2(t_lo + i, r);
+    }
+}
+
+// one CTA per request
+__global__ void __launch_bounds__(SHARE_THREADS) match_share_kernel(
+    const u64* __restrict__ hash_off, u32 R, const u32* __restrict__ leader, const u32* __restrict__ lcp, u32* first_miss,
+    u32* max_hit, u32* host_hits, u32* k_total, u32* n_gpu, u32* hit_loc, const cw_slot* __restrict__ table, u64 mask,
+    const u64* __restrict__ hashes, u32* list_n) {
+    if (hash_off[R] - hash_off[0] > 0xFFFFFFFFull) return;  // rejected by the probe kernel: outputs and scratch untouched
+    const u32 tid = threadIdx.x, lane = tid & 31;
+    const u32 r = blockIdx.x;
+    const u64 h0 = hash_off[r];
+    const u32 n_r = (u32)(hash_off[r + 1] - h0);
+    const u32 L = lcp[r];
+    const bool follower = L != 0xFFFFFFFFu;
+    u64 lh0 = 0;
+    u32 k_l = 0;
+    if (follower) {
+        const u32 l = leader[r];
+        lh0 = hash_off[l];
+        k_l = min(first_miss[l], (u32)(hash_off[l + 1] - lh0));
+    }
+    // ---- (1) k_total / n_gpu (warp 0)
+    if (tid < 32) {
+        // the leader's run ends inside the shared prefix: so does this one; else it goes on into the own tail
+        const u32 k = !follower ? min(first_miss[r], n_r) : (k_l < L ? k_l : min(first_miss[r], n_r));
+        const u32 own_from = follower ? L : 0u;
+        u32 hh = host_hits[r];
+        if (follower) hh |= host_hits[leader[r]];
+        u32 host_in_run = 0;
+        if (hh) {  // count host-tier blocks inside the run (re-probe when the caller did not ask for hit_loc)
+            for (u32 j = lane; j < k; j += 32) {
+                u32 loc;
+                const u64 at = j < own_from ? lh0 + j : h0 + j;
+                if (hit_loc) loc = hit_loc[at];
+                else table_find(table, mask, cw_remap_key(hashes[at]), &loc);
+                host_in_run += (loc != CW_MISS && (loc & CW_HOST_BIT)) ? 1 : 0;
+            }
+#pragma unroll
+            for (int m = 16; m; m >>= 1) host_in_run += __shfl_xor_sync(0xffffffffu, host_in_run, m);
+        }
+        const u32 mh = max_hit[r];
+        if (hit_loc && mh > max(k, own_from))  // resident blocks of the probed part behind the run's end
+            for (u32 j = max(k, own_from) + lane; j < mh; j += 32) hit_loc[h0 + j] = CW_MISS;
+        if (lane == 0) {
+            k_total[r] = k;
+            n_gpu[r] = k - host_in_run;
+        }
+    }
+    // ---- (2) positions [0, L) of a follower: the leader's locations up to the end of the leader's run, MISS behind
+    if (follower && hit_loc) {
+        const u32* src = hit_loc + lh0;
+        u32* dst = hit_loc + h0;
+        for (u32 j0 = 0; j0 < L; j0 += SHARE_UNROLL * SHARE_THREADS) {
+            u32 v[SHARE_UNROLL];
+#pragma unroll
+            for (int q = 0; q < SHARE_UNROLL; ++q)  // unconditional loads at clamped positions, in flight together
+                v[q] = __ldcg(src + min(j0 + tid + q * SHARE_THREADS, L - 1));
+#pragma unroll
+            for (int q = 0; q < SHARE_UNROLL; ++q) {
+                const u32 j = j0 + tid + q * SHARE_THREADS;
+                if (j < L) __stcs(dst + j, j < k_l ? v[q] : CW_MISS);
+            }
+        }
+    }
+    // ---- (3) the list is consumed (by the probe kernel, in front of this one): empty it for the next call
+    if (r == 0 && tid == 0) *list_n = 0;
 }
 
 __global__ void blocks_update_kernel(const u32* ids, u32 n, u32 size, const u32* session, const u32* depth,
@@ -673,12 +831,41 @@ int32_t cwi_match_prefix(cw_ctx* ctx, const u64* d_hashes, const u64* d_hash_off
     if (blocks < 1) blocks = 1;
     match_probe_kernel<<<(u32)blocks, MATCH_THREADS, 0, ctx->s_main>>>(ctx->table, (u32)mask, d_hashes, d_hash_off, R,
                                                              ctx->m_first_miss, ctx->m_max_hit, ctx->m_host_hits,
-                                                             d_hit_loc, ctx->d_status);
+                                                             d_hit_loc, ctx->d_status, nullptr, nullptr, nullptr);
     CW_LAUNCH_CHECK(ctx);
     match_finish_kernel<<<cdiv((u64)R * 32, 256), 256, 0, ctx->s_main>>>(d_hash_off, R, ctx->m_first_miss,
                                                                          ctx->m_max_hit, ctx->m_host_hits, d_k_total,
                                                                          d_n_gpu, d_hit_loc, ctx->table, mask,
                                                                          d_hashes);
+    CW_LAUNCH_CHECK(ctx);
+    return CW_OK;
+}
+
+int32_t cwi_match_prefix_shared(cw_ctx* ctx, const u64* d_hashes, const u64* d_hash_off, u32 R, const u32* d_leader,
+                                u32* d_k_total, u32* d_n_gpu, u32* d_hit_loc) {
+    if (!R) return CW_OK;
+    const u64 mask = ctx->n_slots - 1;
+    const u32 mr = ctx->cfg.max_requests;
+    u32 *first_miss = ctx->m_shared, *max_hit = ctx->m_shared + mr, *host_hits = ctx->m_shared + 2 * (size_t)mr;
+    u32 *lcp = ctx->m_shared + 3 * (size_t)mr, *list_n = ctx->m_shared + 4 * (size_t)mr;
+    uint2* list = reinterpret_cast<uint2*>(ctx->m_list);
+    match_lcp_kernel<<<cdiv((u64)R * 32, 256), 256, 0, ctx->s_main>>>(d_hashes, d_hash_off, R, d_leader, lcp, list, list_n,
+                                                                      first_miss, max_hit, host_hits);
+    CW_LAUNCH_CHECK(ctx);
+    // one resident wave: the list is short (the leaders' tasks and one tail task per follower) and its length is
+    // known to the device only
+    u64 warps = (ctx->cfg.max_hashed_blocks + CWM_CHUNK - 1) / CWM_CHUNK;
+    u64 blocks = (warps + MATCH_THREADS / 32 - 1) / (MATCH_THREADS / 32);
+    u64 cap = (u64)ctx->n_sm * MATCH_MIN_CTAS;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    match_probe_kernel<<<(u32)blocks, MATCH_THREADS, 0, ctx->s_main>>>(ctx->table, (u32)mask, d_hashes, d_hash_off, R,
+                                                                       first_miss, max_hit, host_hits, d_hit_loc,
+                                                                       ctx->d_status, lcp, list, list_n);
+    CW_LAUNCH_CHECK(ctx);
+    match_share_kernel<<<R, SHARE_THREADS, 0, ctx->s_main>>>(d_hash_off, R, d_leader, lcp, first_miss, max_hit, host_hits,
+                                                             d_k_total, d_n_gpu, d_hit_loc, ctx->table, mask, d_hashes,
+                                                             list_n);
     CW_LAUNCH_CHECK(ctx);
     return CW_OK;
 }

@@ -15,13 +15,16 @@ from harness import gen
 pytestmark = pytest.mark.gpu
 
 
-def test_full_size_step_matches_the_oracle_everywhere():
+@pytest.mark.parametrize("shared_match", [True, False])
+def test_full_size_step_matches_the_oracle_everywhere(shared_match):
+    """shared_match: stage 2a through cw_match_prefix_shared (the bench's step: the queue carries session ids, the
+    leader hint is the longest queued request of the session) or through the plain cw_match_prefix."""
     import torch
 
     from harness import stress
     snap = gen.stress_snapshot(seed=3)
     stream = torch.cuda.Stream()
-    st = stress.StressStep(snap, stream)
+    st = stress.StressStep(snap, stream, shared_match=shared_match)
     S, L = snap.streams.shape
     with torch.cuda.stream(stream):
         pool_sum = int(st.pool.view(torch.int64).sum().item())

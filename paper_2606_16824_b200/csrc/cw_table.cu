@@ -315,12 +315,11 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
                                                           const u64* __restrict__ hashes,
                                                           const u64* __restrict__ hash_off, u32 R, u32* first_miss,
                                                           u32* max_hit, u32* host_hits, u32* hit_loc, u32* status,
-                                                          const u32* __restrict__ lcp, const uint2* __restrict__ list,
+                                                          const uint2* __restrict__ list,
                                                           const u32* __restrict__ list_n) {
-    // lcp (cw_match_prefix_shared only, else NULL): request r is probed from position lcp[r] on (~0: from 0); the
-    // positions in front of it are answered from its leader's results by match_share_kernel; list[0 .. *list_n) are
-    // the tasks that hold at least one position to probe (in no particular order), each with the request its first
-    // position lies in (what the search below would find)
+    // list (cw_match_prefix_shared only, else NULL): the tasks to probe, in no particular order, as (request, first
+    // position inside the request) pairs: up to CWM_CHUNK positions of ONE request each, so every task takes the
+    // lane-independent path below; the plain call walks the flat CSR in CWM_CHUNK-aligned tasks instead
     __shared__ u64 s_key[MATCH_THREADS / 32][CWM_CHUNK];
     __shared__ u32 s_loc[MATCH_THREADS / 32][CWM_CHUNK];
     // hash_off may be a slice of a longer CSR array: positions below are 32-bit offsets from its first hash
@@ -339,11 +338,11 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
     // answered without touching the table (the leading run is over); a miss recorded by an earlier task of the
     // same request is honoured too when the warp enters that request
     for (u32 wi = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; wi < n_tasks; wi += nwarps) {
-        uint2 le = make_uint2(wi, 0u);
+        uint2 le = make_uint2(0u, 0u);
         if (list) le = list[wi];
-        const u32 c0 = le.x * CWM_CHUNK;
-        // largest r with hash_off[r] <= c0 (r < R), 32-ary search, warp-uniform, once per task
-        u32 lo = le.y, hi = list ? lo + 1 : R;
+        u32 c0 = wi * CWM_CHUNK;
+        // largest r with hash_off[r] <= c0 (r < R), 32-ary search, warp-uniform, once per task (a listed task names it)
+        u32 lo = le.x, hi = list ? lo + 1 : R;
         while (hi - lo > 1) {
             u32 step = (hi - lo + 31) >> 5;
             u32 p = lo + lane * step;
@@ -356,21 +355,14 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
         u32 r_base = lo;  // request of the first hash of the current round (kept up to date below)
         u32 req_start = (u32)(hash_off[lo] - h_first), req_end = (u32)(hash_off[lo + 1] - h_first);
         u32 dead_r = 0xFFFFFFFFu, checked_r = 0xFFFFFFFFu;  // request known to have missed / whose global state was read
-        const u32 c1 = min(total, c0 + CWM_CHUNK);
+        if (list) c0 = req_start + le.y;
+        const u32 c1 = list ? min(req_end, c0 + CWM_CHUNK) : min(total, c0 + CWM_CHUNK);
         if (c1 <= req_end) {
             // ---- the whole task lies inside request r_base (the common case): LANE-INDEPENDENT probing.  Lane l
             // owns the hashes c0 + l + 32k (coalesced) and walks them front to back on its own, one slot load per
             // iteration of a warp-synchronous loop, so the warp waits for the longest SUM of probe lengths over a
             // lane's keys instead of the sum over rounds of the longest probe of the round.
             const u32 j0 = c0 - req_start;
-            u32 skip = 0;  // leading positions of the task that belong to the shared prefix (not probed here)
-            if (lcp) {
-                const u32 from = lcp[r_base];
-                if (from != 0xFFFFFFFFu) {
-                    if (from >= j0 + (c1 - c0)) continue;  // the whole task is answered from the leader
-                    skip = from > j0 ? from - j0 : 0u;
-                }
-            }
             if (j0 > 0 && __ldcg(first_miss + r_base) < j0) {  // an earlier task of the request already missed
                 if (hl)
                     for (u32 g = c0 + lane; g < c1; g += 32) __stcs(hl + g, CW_MISS);
@@ -391,9 +383,8 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
                 for (int q = 0; q < KPL; ++q) wkey[lane + 32 * q] = cw_remap_key(kk[q]);  // read back by this lane only
             }
             u32 pos = lane;          // position of this lane's current key inside the task
-            if (skip > lane) pos += (skip - lane + 31) & ~31u;  // first position of this lane at or behind `skip`
             u32 limit = n_task;      // warp-uniform: min(n_task, first missing position seen so far)
-            uint2 key = *reinterpret_cast<const uint2*>(wkey + (pos & (CWM_CHUNK - 1)));
+            uint2 key = *reinterpret_cast<const uint2*>(wkey + pos);
             const u32 pmask = mask >> 1;          // the table as pairs of slots: one 32-byte sector each
             u32 pair = (key.x & mask) >> 1;       // homes are even slots
             for (;;) {
@@ -431,14 +422,14 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
 #pragma unroll
             for (int q = 0; q < KPL; ++q) {
                 const u32 p = lane + 32 * q;
-                const u32 l = (p < limit && p >= skip) ? wloc[p] : CW_MISS;
+                const u32 l = p < limit ? wloc[p] : CW_MISS;
                 host += (l != CW_MISS && (l & CW_HOST_BIT)) ? 1u : 0u;
-                if (hl && p < n_task && p >= skip) __stcs(hl + c0 + p, l);  // streaming: not re-read by this kernel
+                if (hl && p < n_task) __stcs(hl + c0 + p, l);  // streaming: hit_loc is not re-read by this kernel
             }
             host = __reduce_add_sync(0xffffffffu, host);
             if (lane == 0) {
                 if (limit < n_task) atomicMin(&first_miss[r_base], j0 + limit);
-                if (limit > skip) atomicMax(&max_hit[r_base], j0 + limit);
+                if (limit) atomicMax(&max_hit[r_base], j0 + limit);
                 if (host) atomicAdd(&host_hits[r_base], host);
             }
             __syncwarp();  // the staging rows are reused by the next task of this warp
@@ -452,7 +443,7 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
                 req_end = (u32)(hash_off[r_base + 1] - h_first);
             }
             const u32 g = g0 + lane;
-            bool active = g < c1;
+            const bool active = g < c1;
             const u64 key = key_next;
             if (g + 32 < c1) key_next = hs[g + 32];  // prefetch the next round
             u32 r = r_base;
@@ -463,10 +454,6 @@ __global__ void __launch_bounds__(MATCH_THREADS, MATCH_MIN_CTAS) match_probe_ker
                     while (g >= (u32)(hash_off[r + 1] - h_first)) ++r;
                 j = active ? g - (u32)(hash_off[r] - h_first) : 0;
                 uniform = __all_sync(0xffffffffu, !active || r == r_base);
-            }
-            if (lcp && active) {  // positions of the shared prefix are not probed here
-                const u32 from = lcp[r];
-                if (from != 0xFFFFFFFFu && j < from) active = false;
             }
             if (uniform) {
                 if (r_base != checked_r && r_base != dead_r) {  // entering a request: did an earlier task miss?
@@ -549,9 +536,10 @@ __global__ void __launch_bounds__(256) match_finish_kernel(const u64* __restrict
 // (say the longest queued request of the session).  Because the hashes are CHAIN hashes (stage 1: H_j is a function of
 // the whole token prefix), two requests that agree at position p agree at every position before p, so
 //   match_lcp_kernel    finds L_r = number of leading hashes request r shares with its leader by a 32-ary search
-//                       (three rounds for 8192 blocks) without touching the table, and appends the 128-position
-//                       tasks that still hold something to probe to a compact list,
-//   match_probe_kernel  walks that list: leaders in full, every other request from position L_r on (its own tail),
+//                       (three rounds for 8192 blocks) without touching the table, and appends the request's tasks
+//                       (128 positions each, from position 0 of a leader, from L_r of a follower) to a compact list,
+//   match_probe_kernel  walks that list: leaders in full, every other request from position L_r on (its own tail);
+//                       a listed task lies inside one request, so all of them take the lane-independent path,
 //   match_share_kernel  (one CTA per request) answers positions [0, L_r) of a follower from the leader's results,
 //                       computes k_total / n_gpu and resets the list counter.
 // A hint that shares nothing (or is not itself a leader) only costs the search: the request is probed on its own.
@@ -601,16 +589,15 @@ __global__ void __launch_bounds__(256) match_lcp_kernel(const u64* __restrict__ 
         max_hit[r] = 0;
         host_hits[r] = 0;
     }
-    // the tasks whose FIRST position lies in this request, minus those that end inside the shared prefix
-    const u32 start = (u32)(a0 - h_first), end = (u32)(a1 - h_first);
-    const u32 t_hi = (end + CWM_CHUNK - 1) / CWM_CHUNK;
-    u32 t_lo = (start + CWM_CHUNK - 1) / CWM_CHUNK;
-    if (out != 0xFFFFFFFFu) t_lo = max(t_lo, (start + out) / CWM_CHUNK);
-    if (t_hi > t_lo) {
+    // the tasks of this request: CWM_CHUNK positions each, from position 0 (leader) or L (follower: its own tail) on
+    const u32 n_r = (u32)(a1 - a0);
+    const u32 from = out == 0xFFFFFFFFu ? 0u : out;
+    const u32 n_t = (n_r - from + CWM_CHUNK - 1) / CWM_CHUNK;
+    if (n_t) {
         u32 base = 0;
-        if (lane == 0) base = atomicAdd(list_n, t_hi - t_lo);
+        if (lane == 0) base = atomicAdd(list_n, n_t);
         base = __shfl_sync(0xffffffffu, base, 0);
-        for (u32 i = lane; i < t_hi - t_lo; i += 32) list[base + i] = make_uint2(t_lo + i, r);
+        for (u32 i = lane; i < n_t; i += 32) list[base + i] = make_uint2(r, from + i * CWM_CHUNK);
     }
 }
 
@@ -831,7 +818,7 @@ int32_t cwi_match_prefix(cw_ctx* ctx, const u64* d_hashes, const u64* d_hash_off
     if (blocks < 1) blocks = 1;
     match_probe_kernel<<<(u32)blocks, MATCH_THREADS, 0, ctx->s_main>>>(ctx->table, (u32)mask, d_hashes, d_hash_off, R,
                                                              ctx->m_first_miss, ctx->m_max_hit, ctx->m_host_hits,
-                                                             d_hit_loc, ctx->d_status, nullptr, nullptr, nullptr);
+                                                             d_hit_loc, ctx->d_status, nullptr, nullptr);
     CW_LAUNCH_CHECK(ctx);
     match_finish_kernel<<<cdiv((u64)R * 32, 256), 256, 0, ctx->s_main>>>(d_hash_off, R, ctx->m_first_miss,
                                                                          ctx->m_max_hit, ctx->m_host_hits, d_k_total,
@@ -861,7 +848,7 @@ int32_t cwi_match_prefix_shared(cw_ctx* ctx, const u64* d_hashes, const u64* d_h
     if (blocks < 1) blocks = 1;
     match_probe_kernel<<<(u32)blocks, MATCH_THREADS, 0, ctx->s_main>>>(ctx->table, (u32)mask, d_hashes, d_hash_off, R,
                                                                        first_miss, max_hit, host_hits, d_hit_loc,
-                                                                       ctx->d_status, lcp, list, list_n);
+                                                                       ctx->d_status, list, list_n);
     CW_LAUNCH_CHECK(ctx);
     match_share_kernel<<<R, SHARE_THREADS, 0, ctx->s_main>>>(d_hash_off, R, d_leader, lcp, first_miss, max_hit, host_hits,
                                                              d_k_total, d_n_gpu, d_hit_loc, ctx->table, mask, d_hashes,

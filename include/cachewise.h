@@ -217,9 +217,9 @@ int32_t cw_score_evict(cw_ctx* ctx, uint32_t tick_now, uint32_t S, uint32_t F, c
  * the output arrays must not be touched between begin and end.  One begin may be outstanding per ctx (a second one,
  * or an end without a begin, returns CW_E_STATE).  Both calls can be captured into one CUDA graph on stream_main (the
  * side stream joins the capture as a parallel branch).
- *   n_ctas: how many CTAs (= SMs) the speculative kernel may occupy; 0 = library default (a quarter of the SMs:
- *   measured on configs[2], 37 of 148 CTAs is where the steady step is shortest — the kernels on stream_main keep
- *   the other three quarters of the machine and both branches end together). */
+ *   n_ctas: how many CTAs (= SMs) the speculative kernel may occupy; 0 = library default (a third of the SMs:
+ *   measured on configs[2], 44 to 56 of 148 CTAs is where the steady step is shortest — the kernels on stream_main
+ *   keep the other two thirds of the machine and both branches end together). */
 int32_t cw_score_evict_begin(cw_ctx* ctx, uint32_t tick_now, uint32_t S, uint32_t F, const uint8_t* d_features,
                              const int16_t* d_weights, int32_t bias, const uint8_t* d_session_state,
                              const uint32_t* d_tau_override, uint32_t tier, uint32_t* d_victims,

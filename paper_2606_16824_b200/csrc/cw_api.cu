@@ -341,7 +341,7 @@ int32_t cw_score_evict_begin(cw_ctx* ctx, uint32_t tick_now, uint32_t S, uint32_
     // fork: the side stream starts after everything queued on stream_main so far
     CW_CUDA(ctx, cudaEventRecord(ctx->ev_fork, ctx->s_main));
     CW_CUDA(ctx, cudaStreamWaitEvent(ctx->s_side, ctx->ev_fork, 0));
-    st = cwi_score_evict(ctx, ctx->s_side, n_ctas ? n_ctas : (u32)(ctx->n_sm + 3) / 4, tick_now, S, F, d_features,
+    st = cwi_score_evict(ctx, ctx->s_side, n_ctas ? n_ctas : (u32)(ctx->n_sm + 2) / 3, tick_now, S, F, d_features,
                          d_weights, bias, d_session_state, d_tau_override, nullptr, tier, d_victims, d_victim_scores,
                          ctx->spec_n, cap);
     if (st) return st;

@@ -15,11 +15,17 @@ MISS, HOST = 0xFFFFFFFF, 0x80000000
 def _shared(ctx, h, hoff, leader, want_loc=True):
     from gpu_util import dev, host, zeros
     R = hoff.size - 1
-    k, g, loc = zeros(R, np.uint32), zeros(R, np.uint32), zeros(h.size, np.uint32)
-    loc.fill_(0x5A5A5A5A)                                   # every position must be written
-    ctx.match_prefix_shared(dev(h), dev(hoff), R, dev(np.asarray(leader, np.uint32)), k, g, loc if want_loc else None)
+    G = 32                                                  # guard words around every output
+    k, g, loc = zeros(R + 2 * G, np.uint32), zeros(R + 2 * G, np.uint32), zeros(h.size + 2 * G, np.uint32)
+    for t in (k, g, loc):
+        t.fill_(0x5A5A5A5A)                                 # every position must be written, nothing beside them
+    ctx.match_prefix_shared(dev(h), dev(hoff), R, dev(np.asarray(leader, np.uint32)), k[G:], g[G:],
+                            loc[G:] if want_loc else None)
     assert ctx.sync(check=False) == 0
-    return host(k, np.uint32)[:R], host(g, np.uint32)[:R], host(loc, np.uint32)[:h.size]
+    hk, hg, hl = host(k, np.uint32), host(g, np.uint32), host(loc, np.uint32)
+    for a, n in ((hk, R), (hg, R), (hl, h.size)):
+        assert (a[:G] == 0x5A5A5A5A).all() and (a[G + n:] == 0x5A5A5A5A).all(), "write outside an output array"
+    return hk[G:G + R], hg[G:G + R], hl[G:G + h.size]
 
 
 def _flat(ctx, h, hoff):
@@ -129,3 +135,39 @@ def test_shared_match_followers_longer_than_the_leader_and_resident_tails():
         if resident_upto == 700:
             assert ek.tolist() == [400, 530, 130, 400, 0, 700, 390, 0]
         ctx.close()
+
+
+def test_shared_match_on_a_slice_of_a_longer_csr():
+    """hash_off may be a slice of a longer CSR array (absolute offsets), as for cw_match_prefix: requests [a, b) of the
+    queue, leader indices relative to the slice, outputs at the absolute positions of d_hit_loc."""
+    from gpu_util import dev, host, small_ctx, zeros
+    from test_gpu_match_schedule import _insert
+    S, L, RB = 6, 8192, 256
+    snap = gen.stress_snapshot(seed=9, S=S, L=L, RB=RB, req_per_session=10, len_median=2500, len_min=16, len_max=L)
+    ctx = small_ctx(num_blocks=snap.M, table_log2_slots=snap.table_log2, max_hashed_blocks=1 << 20)
+    hs, _ = oracle.hash_blocks(snap.streams.reshape(-1), gen.stream_tok_off(S, L))
+    hs = hs.reshape(S, L // 16)[:, :RB].reshape(-1)
+    loc = np.arange(S * RB, dtype=np.uint32)
+    ot = oracle.Table(snap.table_log2)
+    ot.insert(hs, loc)
+    _insert(ctx, hs, loc)
+    h, hoff = oracle.hash_blocks(snap.tokens, snap.tok_off)
+    n = (hoff[1:] - hoff[:-1]).astype(np.int64)
+    ek, eg, eloc = ot.match_prefix(h, hoff)
+    lead = _longest_of_session(snap.req_session, n)
+    a, b = 13, 47                                           # cuts sessions 1 and 4 in two
+    sl = lead[a:b].astype(np.int64) - a
+    sl[(sl < 0) | (sl >= b - a)] = np.arange(b - a)[(sl < 0) | (sl >= b - a)]      # leader outside the slice: own
+    R = b - a
+    k, gg = zeros(R, np.uint32), zeros(R, np.uint32)
+    d_loc = zeros(h.size, np.uint32)
+    d_loc.fill_(0x5A5A5A5A)
+    d_hoff = dev(hoff)
+    ctx.match_prefix_shared(dev(h), d_hoff[a:], R, dev(sl.astype(np.uint32)), k, gg, d_loc)
+    assert ctx.sync(check=False) == 0
+    assert (host(k, np.uint32)[:R] == ek[a:b]).all() and (host(gg, np.uint32)[:R] == eg[a:b]).all()
+    got = host(d_loc, np.uint32)[:h.size]
+    lo, hi = int(hoff[a]), int(hoff[b])
+    assert (got[lo:hi] == eloc[lo:hi]).all()
+    assert (got[:lo] == 0x5A5A5A5A).all() and (got[hi:] == 0x5A5A5A5A).all()
+    ctx.close()

@@ -654,10 +654,18 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
             const DigitPlan& pn = s_plan2;
             u64 m_or_hi = 0, m_nand_hi = 0, v_or_hi = 0, v_nand_hi = 0;  // next candidate set / victims
             u32 m_or_lo = 0, m_nand_lo = 0, v_or_lo = 0, v_nand_lo = 0;
-            for (u32 tile = blockIdx.x; (u64)tile * CWE_MTILE < a.M; tile += G) {
+            // The tiles of this pass cost very different amounts (a tile of an idle session appends 4096 entries, most
+            // tiles nothing), and a pool that keeps a session's blocks together hands whole tiles of one kind to one
+            // CTA: behind the first tile the CTAs therefore draw tickets.  The ticket of the NEXT tile is requested
+            // before the current one is processed (its round trip hides behind the tile) and handed round at the end.
+            __shared__ u32 s_next_tile;
+            u32 tile = blockIdx.x;
+            while ((u64)tile * CWE_MTILE < a.M) {
                 bool f0[CWE_MI], f1[CWE_MI];
                 u32 p0[CWE_MI], p1[CWE_MI];
                 u64 sc[CWE_MI];
+                u32 nxt = 0;
+                if (tid == 0) nxt = G + atomicAdd(&st->tile_cursor, 1u);
                 load_tile(tile);
 #pragma unroll
                 for (int k = 0; k < CWE_MI; ++k) {
@@ -688,20 +696,25 @@ __global__ void __launch_bounds__(CWE_THREADS, 1) evict_kernel(const EvictArgs a
                     bool any = false;
 #pragma unroll
                     for (int k = 0; k < CWE_MI; ++k) any |= f0[k] | f1[k];
-                    if (!__syncthreads_or(any)) continue;
-                }
-                tile_append(f0, f1, p0, p1, &st->n_out, &st->n_cand[1], s_w0, s_w1, s_base);
+                    if (__syncthreads_or(any)) {
+                        tile_append(f0, f1, p0, p1, &st->n_out, &st->n_cand[1], s_w0, s_w1, s_base);
 #pragma unroll
-                for (int k = 0; k < CWE_MI; ++k) {
-                    const u32 b = tile * CWE_MTILE + tid * CWE_MI + k;
-                    if (f0[k]) {
-                        a.out_score[p0[k]] = sc[k];
-                        a.out_id[p0[k]] = b;
-                    } else if (f1[k]) {
-                        a.cand_score[1][p1[k]] = sc[k];
-                        a.cand_id[1][p1[k]] = b;
+                        for (int k = 0; k < CWE_MI; ++k) {
+                            const u32 b = tile * CWE_MTILE + tid * CWE_MI + k;
+                            if (f0[k]) {
+                                a.out_score[p0[k]] = sc[k];
+                                a.out_id[p0[k]] = b;
+                            } else if (f1[k]) {
+                                a.cand_score[1][p1[k]] = sc[k];
+                                a.cand_id[1][p1[k]] = b;
+                            }
+                        }
                     }
                 }
+                if (tid == 0) s_next_tile = nxt;
+                __syncthreads();
+                tile = s_next_tile;
+                __syncthreads();
             }
             stamp(st, n_stamp);  // CTA 0 done with its filter tiles
             if (next) flush_hist(s_hist, a.hist + CWE_BINS);

@@ -94,7 +94,7 @@ struct cw_evict_state {  // all zero between calls, except the barrier words
     u64 tau_masks;                    // OR of (TAU_MAX-tau) << 32 | OR of its complement (global-tau path)
     u64 all_or_hi, all_nand_hi;       // OR of the scores of ALL evictable blocks / of their complements (level-1 plan)
     u32 all_or_lo, all_nand_lo;       // same for the ids
-    u32 cursor0, pad3;                // append cursor of the small-pool materialisation pass
+    u32 cursor0, tile_cursor;         // append cursor of the small-pool materialisation pass; tile tickets of the filter pass
     u32 n_cand[CWE_PASSES + 1];       // candidates of every level
     u32 pad1;
     u32 or_lo[CWE_PASSES + 1], nand_lo[CWE_PASSES + 1];  // OR of the ids / of their complements, per level

@@ -78,7 +78,7 @@ def ncu_traffic():
 
 def ncu_kernel_us():
     """{stage: device time (us) of the stage's main kernel ALONE} from the same committed capture (cold cache,
-    serialised by ncu): context beside the live stage times, which are whole calls (e.g. plan kernel + hash kernel)."""
+    serialised by ncu): context beside the live stage times, which are whole calls (launch and drain included; several kernels for the match)."""
     try:
         head, units, rows = _ncu_rows()
         ki, ti = head.index("Kernel Name"), head.index("gpu__time_duration.sum")

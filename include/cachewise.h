@@ -116,10 +116,10 @@ int32_t cw_hash_blocks(cw_ctx* ctx, const int32_t* d_tokens, const uint64_t* d_t
 
 /* cw_hash_blocks without a ctx and WITHOUT ANY ALLOCATION — for callers that cannot call cudaMalloc (code under CUDA
  * graph capture, tight serving loops, harnesses that forbid it) and therefore cannot cw_create.  Same operation, same
- * kernels and same argument meaning as cw_hash_blocks (stage 1, reading R1); the scratch a ctx would own
- * (unit offsets, plan words, per-CTA hand-over records) is a fixed file-scope device array of about 164 KiB that every
- * GPU loading the library holds until the process exits.  The call issues one 16-byte cudaMemsetAsync and one or two
- * kernels on `stream`, on the CURRENT device; it calls no cudaMalloc / cudaFree / allocating routine.
+ * kernel and same argument meaning as cw_hash_blocks (stage 1, reading R1); the scratch a ctx would own
+ * (ticket / epoch words, per-CTA hand-over records) is a fixed file-scope device array of about 32 KiB that every
+ * GPU loading the library holds until the process exits.  The call issues one 16-byte cudaMemsetAsync and one
+ * kernel on `stream`, on the CURRENT device; it calls no cudaMalloc / cudaFree / allocating routine.
  *   R                  at most CW_HASH_STATIC_MAX_REQUESTS, else CW_E_INVAL (and a line on stderr); 0 = no-op
  *   max_hashed_blocks  capacity of d_hashes in blocks: hash_off[R]-hash_off[0] beyond it is reported, nothing written
  *   d_status           uint32 device word or NULL: device-detected conditions (the ones cw_hash_blocks reports at

@@ -44,7 +44,6 @@ void free_all(cw_ctx* c) {
     cudaFree(c->dbg_stamps);
     cudaFree(c->d_status);
     if (c->h_status) cudaFreeHost(c->h_status);
-    cudaFree(c->hash_unit_off);
     cudaFree(c->hash_plan);
     cudaFree(c->hash_rec);
     cudaFree(c->m_first_miss);
@@ -129,7 +128,6 @@ int32_t cw_create(const cw_config* cfg, cw_ctx** out) {
     *c->h_status = 0;
     // stage 1
     c->hash_grid = cwi_hash_grid(c->n_sm);
-    CW_CUDA(c, dalloc_zero(&c->hash_unit_off, (size_t)cfg->max_requests + 1, s));
     CW_CUDA(c, dalloc_zero(&c->hash_plan, 4, s));
     CW_CUDA(c, dalloc_zero(&c->hash_rec, (size_t)c->hash_grid, s));
     // stage 2a

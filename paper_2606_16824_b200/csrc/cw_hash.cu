@@ -12,7 +12,7 @@
 //          warp of unit i to the warp of unit i+1 through a shared-memory ring (one mbarrier per slot): the serial
 //          part per unit is one multiply-add, everything else of a unit runs beside the other warps' units
 //   grid : the list of units (request-aligned runs of <= 256 blocks) is cut into gridDim.x CONTIGUOUS ranges
-//          of equal length, one per CTA.  A CTA therefore walks its requests sequentially and never waits on
+//          of about equal length (equal in tokens), one per CTA.  A CTA therefore walks its requests sequentially and never waits on
 //          another CTA (no look-back, no spinning).  Only the first request of a range can have begun in an
 //          earlier range: that boundary segment is scanned with carry-in 0 and patched at the very end of the
 //          CTA, H_j += A^(j-j0+1) * carry_in (linear in the carry, mod 2^64), from the chain states the CTAs of the
@@ -21,9 +21,12 @@
 //          CTA that is waited for has always started: the single wait per CTA cannot deadlock and happens
 //          when both CTAs are finishing anyway.
 //
-// Two launches per call (one for calls of at most CWH_SMALL_R requests — the steady-state step — where every CTA of
-// hash_kernel rebuilds the plan in shared memory and the last CTA to finish re-arms the ticket and the epoch):
-//   hash_plan_kernel   units per request -> exclusive scan unit_off[R+1]; validates the offsets
+// One launch per call, no plan pass: the TOKEN space of the call is cut into gridDim.x equal pieces (a multiple of a
+// unit's 4096 tokens each) and every CTA moves the two ends of its piece to the first unit at or behind them by a
+// 32-ary search over tok_off (three rounds for 4096 requests; both ends are mapped by the same function, so the ranges
+// tile the unit list); the offsets of every request are validated once, spread over the grid; the last CTA to finish
+// re-arms the ticket and advances the epoch.  (Rounds 1-2 ran a one-CTA plan kernel first — units per request,
+// exclusive scan, 10 us plus a launch gap in front of an 87 us kernel — and cut the UNIT list into equal ranges.)
 //   hash_kernel        the streaming pass: one producer warp issues ONE TMA bulk copy (cp.async.bulk, L2
 //                      evict-first) of each unit's 16 KiB of token ids into a 4-stage shared-memory ring
 //                      (mbarrier full/empty); a consumer warp reads its unit with conflict-free 16-byte loads (the
@@ -55,13 +58,11 @@ struct HashArgs {
     const u64* salt;
     const u64* hash_off;
     u64* hashes;
-    u64* unit_off;      // [R+1] exclusive scan of units per request
-    u64* plan;          // [0] total units, [1] call epoch, [2] range ticket, [3] CTAs done (small calls)
+    u64* plan;          // [1] call epoch, [2] range ticket, [3] CTAs done ([0] unused)
     cw_hash_rec* rec;   // per CTA of hash_kernel
     u32* status;
     u64 max_hashed;
     u32 R;
-    u32 small;          // R <= CWH_SMALL_R: no plan kernel, every CTA rebuilds the plan in shared memory
 };
 
 enum { MODE_CONTINUE = 0, MODE_SEED = 1, MODE_ZERO = 2 };
@@ -85,8 +86,8 @@ struct __align__(128) HashSmem {
     u64 carry_bar[CWH_WARPS];   // slot i % CWH_WARPS: the chain state after unit i of the range is published
     u64 carry_ring[CWH_WARPS];
     u64 carry_in;
-    u32 uoff[CWH_SMALL_R + 1];  // small calls: exclusive scan of units per request
     u32 wsum[CWH_WARPS + 1];
+    u32 b_r[2], b_t[2];         // the range's two ends as (request, unit inside the request)
     u32 range;
     u32 rec_flags;
     u32 rec_bseg_len;
@@ -104,62 +105,63 @@ __device__ __forceinline__ u64 pow_u64(u64 base, u64 e) {
     return r;
 }
 
-// ------------------------------------------------------------------------------------------------ plan
-__device__ __forceinline__ u64 plan_units(const HashArgs& a, u32 r, bool too_big) {
-    if (too_big) return 0;
+// ------------------------------------------------------------------------------------------------ requests
+// Units (request-aligned runs of <= 256 blocks from start_block on) of request r; ~0 if its offsets are inconsistent.
+// Loads first, decisions after (a load behind a condition is not issued until the condition is known).
+struct ReqInfo {
+    u64 t0, h0, n, sb, units;  // token offset, hash offset, blocks, first block to hash, units (0 if invalid)
+    bool invalid;
+};
+__device__ __forceinline__ ReqInfo req_info(const HashArgs& a, u32 r) {
     const u64 t0 = a.tok_off[r], t1 = a.tok_off[r + 1], h0 = a.hash_off[r], h1 = a.hash_off[r + 1];
     const u64 sb = a.start_block ? a.start_block[r] : 0;
-    if (t1 < t0 || h1 < h0 || (h1 - h0) != ((t1 - t0) >> 4) || sb > h1 - h0) return ~0ull;  // invalid request
-    return (h1 - h0 - sb + CWH_UNIT - 1) >> CWH_UNIT_LOG2;
+    ReqInfo q;
+    q.invalid = t1 < t0 || h1 < h0 || (h1 - h0) != ((t1 - t0) >> 4) || sb > h1 - h0;
+    q.t0 = t0;
+    q.h0 = h0;
+    q.n = h1 - h0;
+    q.sb = sb;
+    q.units = q.invalid ? 0ull : (h1 - h0 - sb + CWH_UNIT - 1) >> CWH_UNIT_LOG2;
+    return q;
 }
 
-__global__ void __launch_bounds__(1024) hash_plan_kernel(const HashArgs a) {
-    __shared__ u64 s_warp[32];
-    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+// A boundary of the token space (token index p, T0 <= p <= TR) -> the first unit at or behind it: (request, unit inside
+// the request); (R, 0) behind the last unit.  Warp-collective: a 32-ary search over tok_off for the request that holds
+// p, then at most a hop over requests without work.  Both ends of a range are mapped by the same function, so the
+// ranges tile the unit list whatever the offsets look like.
+__device__ __forceinline__ void map_boundary(const HashArgs& a, u64 p, u32 lane, u32& r_out, u32& t_out) {
     const u32 R = a.R;
-    const bool too_big = a.hash_off[R] < a.hash_off[0] || a.hash_off[R] - a.hash_off[0] > a.max_hashed;
-    // every thread owns a contiguous run of requests: one round of loads, one block scan
-    const u32 per = (R + 1023) / 1024;
-    const u32 lo = min(R, tid * per), hi = min(R, lo + per);
-    u64 local = 0;
-    bool bad = false;
-    for (u32 r = lo; r < hi; ++r) {
-        const u64 T = plan_units(a, r, too_big);
-        if (T == ~0ull) bad = true;
-        else local += T;
+    u32 lo = 0, hi = R;  // largest r < R with tok_off[r] <= p
+    while (hi - lo > 1) {
+        const u32 step = (hi - lo + 31) >> 5;
+        const u32 q = lo + lane * step;
+        const bool ok = q < hi && a.tok_off[q] <= p;
+        u32 cnt = __popc(__ballot_sync(0xffffffffu, ok));
+        cnt = cnt ? cnt : 1u;  // (tok_off[lo] <= p holds for consistent offsets)
+        const u32 nlo = lo + (cnt - 1) * step;
+        hi = min(hi, nlo + step);
+        lo = nlo;
     }
-    if (bad) atomicOr(a.status, CWS_INVAL);
-    u64 inc = local;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        u64 y = shfl64_up(inc, d);
-        if (lane >= d) inc += y;
+    const ReqInfo q = req_info(a, lo);
+    const u64 hs = q.t0 + 16 * q.sb;  // first token that is hashed
+    const u64 t = p > hs ? (p - hs + (16 * CWH_UNIT - 1)) / (16 * CWH_UNIT) : 0;
+    if (t < q.units) {
+        r_out = lo;
+        t_out = (u32)t;
+        return;
     }
-    if (lane == 31) s_warp[warp] = inc;
-    __syncthreads();
-    if (warp == 0) {
-        u64 w = s_warp[lane], wi = w;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            u64 y = shfl64_up(wi, d);
-            if (lane >= d) wi += y;
-        }
-        s_warp[lane] = wi - w;
-        if (lane == 31) {
-            a.unit_off[R] = wi;
-            a.plan[0] = wi;
-            a.plan[1] = a.plan[1] + 1;  // epoch of this call (ready flags of earlier calls become stale)
-            a.plan[2] = 0;              // range ticket
-            if (too_big) atomicOr(a.status, CWS_INVAL);
+    for (u32 r = lo + 1; r < R; r += 32) {  // the next request with work
+        const u32 rr = r + lane;
+        const bool has = rr < R && req_info(a, min(rr, R - 1)).units > 0;
+        const u32 m = __ballot_sync(0xffffffffu, has);
+        if (m) {
+            r_out = r + (u32)__ffs(m) - 1;
+            t_out = 0;
+            return;
         }
     }
-    __syncthreads();
-    u64 run = s_warp[warp] + inc - local;
-    for (u32 r = lo; r < hi; ++r) {
-        a.unit_off[r] = run;
-        const u64 T = plan_units(a, r, too_big);
-        if (T != ~0ull) run += T;
-    }
+    r_out = R;
+    t_out = 0;
 }
 
 // ------------------------------------------------------------------------------------------------ digests
@@ -208,81 +210,64 @@ __global__ void __launch_bounds__(CWH_THREADS, CWH_MIN_CTAS) hash_kernel(const H
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     if (tid == 0) sm.range = atomicAdd(reinterpret_cast<unsigned int*>(a.plan + 2), 1u);
-    const bool small = a.small != 0;
-    u64 U;
-    u32 epoch;
-    if (small) {
-        // ---- small call (R <= CWH_SMALL_R, the steady-state step): no plan kernel.  Every CTA computes the units of
-        // every request (a few per thread, one round of loads), scans them and keeps the offsets in shared memory; the
-        // last CTA to finish re-arms the ticket and advances the epoch.
-        const u32 R = a.R;
-        const bool too_big = a.hash_off[R] < a.hash_off[0] || a.hash_off[R] - a.hash_off[0] > a.max_hashed;
-        constexpr int PER = (CWH_SMALL_R + CWH_THREADS - 1) / CWH_THREADS;  // requests per thread
-        u32 tu[PER];
+    const u32 R = a.R, G = gridDim.x;
+    const u64 T0 = a.tok_off[0], TR = a.tok_off[R], H0 = a.hash_off[0], HR = a.hash_off[R];
+    const bool too_big = HR < H0 || HR - H0 > a.max_hashed || TR < T0;
+    const u32 epoch = (u32)a.plan[1] + 1;  // advanced by the last CTA to finish (records of earlier calls go stale)
+    {   // every request's offsets are checked once, spread over the grid (the status word is all this produces)
         bool bad = too_big;
-        u32 local = 0;
-#pragma unroll
-        for (int k = 0; k < PER; ++k) {
-            const u32 r = tid * PER + k;
-            u64 T = r < R ? plan_units(a, r, too_big) : 0;
-            if (T == ~0ull) {
-                bad = true;
-                T = 0;
-            }
-            tu[k] = (u32)T;
-            local += (u32)T;
-        }
-        if (bad && blockIdx.x == 0) atomicOr(a.status, CWS_INVAL);
-        u32 inc = local;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const u32 y = __shfl_up_sync(0xffffffffu, inc, d);
-            if (lane >= (u32)d) inc += y;
-        }
-        if (lane == 31) sm.wsum[warp] = inc;
-        __syncthreads();
-        u32 before = 0, total = 0;
-#pragma unroll
-        for (u32 w = 0; w <= CWH_WARPS; ++w) {
-            const u32 v = sm.wsum[w];
-            if (w < warp) before += v;
-            total += v;
-        }
-        u32 run = before + inc - local;
-#pragma unroll
-        for (int k = 0; k < PER; ++k) {
-            const u32 r = tid * PER + k;
-            if (r < R) sm.uoff[r] = run;
-            run += tu[k];
-        }
-        if (tid == 0) sm.uoff[R] = total;
-        U = total;
-        epoch = (u32)a.plan[1] + 1;
-    } else {
-        U = a.plan[0];
-        epoch = (u32)a.plan[1];
+        for (u32 r = blockIdx.x * CWH_THREADS + tid; r < R; r += G * CWH_THREADS) bad |= req_info(a, r).invalid;
+        if (bad) atomicOr(a.status, CWS_INVAL);
     }
     __syncthreads();
-    auto uo = [&](u32 i) -> u64 { return small ? (u64)sm.uoff[i] : a.unit_off[i]; };
-    auto call_done = [&]() {  // self-cleaning: the last CTA re-arms the ticket (a small call may follow without a plan
-        if (tid == 0) {       // kernel) and, in a small call, advances the epoch
+    auto call_done = [&]() {  // self-cleaning: the last CTA to finish re-arms the ticket and advances the epoch
+        if (tid == 0) {
             const u32 old = atomicAdd(reinterpret_cast<unsigned int*>(a.plan + 3), 1u);
-            if (old == gridDim.x - 1) {
+            if (old == G - 1) {
                 a.plan[3] = 0;
                 a.plan[2] = 0;
-                if (small) a.plan[1] = a.plan[1] + 1;
+                a.plan[1] = a.plan[1] + 1;
             }
         }
     };
-    const u32 range = sm.range;  // ranges in ticket order: every lower range belongs to a CTA that has started
-    const u64 per = (U + gridDim.x - 1) / gridDim.x;
-    const u64 u_begin = min(U, per * range), u_end = min(U, u_begin + per);
-    if (u_begin >= u_end) {  // empty range (uniform over the CTA): nobody waits for it
+    // ---- the range of this CTA.  There is no plan pass: the TOKEN space [T0, TR) is cut into G equal pieces (a
+    // multiple of a unit's 4096 tokens each), and a boundary is moved to the first unit at or behind it by a search
+    // over tok_off.  Ranges in ticket order: every lower range belongs to a CTA that has started.
+    const u32 range = sm.range;
+    u64 per_tok = (TR - T0 + G - 1) / G;
+    per_tok = max((per_tok + 16 * CWH_UNIT - 1) / (16 * CWH_UNIT), (u64)1) * (16 * CWH_UNIT);
+    const u64 pb = T0 + (u64)range * per_tok;
+    if (too_big || pb >= TR) {  // nothing to do (uniform over the CTA): nobody waits for an empty range
         call_done();
         return;
     }
+    if (warp < 2) {
+        u32 r, t;
+        map_boundary(a, warp ? min(TR, pb + per_tok) : pb, lane, r, t);
+        if (lane == 0) {
+            sm.b_r[warp] = r;
+            sm.b_t[warp] = t;
+        }
+    }
+    __syncthreads();
+    const u32 r_b = sm.b_r[0], t_b = sm.b_t[0], r_e = sm.b_r[1], t_e = sm.b_t[1];
+    if (r_b == r_e && t_b == t_e) {  // a stretch of tokens without a unit (short or resumed requests)
+        call_done();
+        return;
+    }
+    u32 n_units;
+    {   // units of the requests [r_b, r_e), less the t_b units in front of the range, plus the t_e units of request r_e
+        u32 local = 0;
+        for (u32 r = r_b + tid; r < r_e; r += CWH_THREADS) local += (u32)req_info(a, r).units;
+        local = __reduce_add_sync(0xffffffffu, local);
+        if (lane == 0) sm.wsum[warp] = local;
+        __syncthreads();
+        u32 total = 0;
+#pragma unroll
+        for (u32 w = 0; w <= CWH_WARPS; ++w) total += sm.wsum[w];
+        n_units = total - t_b + t_e;
+    }
 
-    const u32 n_units = (u32)(u_end - u_begin);
     if (tid == 0) {
         for (int s = 0; s < CWH_STAGES; ++s) {
             mbar_init(smem_u32(&sm.full[s]), 1);
@@ -295,36 +280,23 @@ __global__ void __launch_bounds__(CWH_THREADS, CWH_MIN_CTAS) hash_kernel(const H
 
     if (warp == CWH_WARPS) {
         // ------------------------------------------------------------------ producer warp
-        const u32 R = a.R;
-        // largest r with unit_off[r] <= u_begin (=> unit_off[r+1] > u_begin), 32-ary search
-        u32 lo = 0, hi = R;
-        while (hi - lo > 1) {
-            u32 step = (hi - lo + 31) >> 5;
-            u32 p = lo + lane * step;
-            bool ok = p < hi && uo(p) <= u_begin;
-            u32 cnt = __popc(__ballot_sync(0xffffffffu, ok));
-            u32 nlo = lo + (cnt - 1) * step;
-            hi = min(hi, nlo + step);
-            lo = nlo;
-        }
         if (lane == 0) {
             const u64 policy = policy_evict_first();
-            u32 r = lo;
-            u64 u = u_begin;
-            u64 uo0 = uo(r), uo1 = uo(r + 1);
-            u64 t = u - uo0;
+            u32 r = r_b;
+            u64 t = t_b;
             const bool starts_mid = t > 0;  // the first request began in an earlier CTA's range
             bool in_bseg = starts_mid;
             u64 bseg_first = 0, bseg_len = 0;
-            u64 h0 = 0, n_r = 0, t0 = 0, sb = 0, seed = 0;
+            u64 h0 = 0, n_r = 0, t0 = 0, sb = 0, seed = 0, un = 0;
             bool fresh = true;
-            u32 it = 0;
-            for (; u < u_end; ++u, ++it) {
+            for (u32 it = 0; it < n_units; ++it) {
                 if (fresh) {
-                    h0 = a.hash_off[r];
-                    n_r = a.hash_off[r + 1] - h0;
-                    t0 = a.tok_off[r];
-                    sb = a.start_block ? a.start_block[r] : 0;
+                    const ReqInfo q = req_info(a, r);
+                    h0 = q.h0;
+                    n_r = q.n;
+                    t0 = q.t0;
+                    sb = q.sb;
+                    un = q.units;
                     seed = sb > 0 ? a.start_state[r] : cw_fin((a.salt ? a.salt[r] : 0ull) ^ CW_K7);
                     fresh = false;
                 }
@@ -335,12 +307,12 @@ __global__ void __launch_bounds__(CWH_THREADS, CWH_MIN_CTAS) hash_kernel(const H
                 ui.valid = 1;
                 ui.nblk = (u32)min((u64)CWH_UNIT, n_r - j0);
                 ui.mis = (u32)(t0 & 3);
-                ui.mode = t == 0 ? MODE_SEED : (u == u_begin ? MODE_ZERO : MODE_CONTINUE);
+                ui.mode = t == 0 ? MODE_SEED : (it == 0 ? MODE_ZERO : MODE_CONTINUE);
                 ui.out_base = h0 + j0;
                 ui.seed = seed;
-                ui.last = (u + 1 == u_end) ? 1u : 0u;
+                ui.last = (it + 1 == n_units) ? 1u : 0u;
                 if (in_bseg) {
-                    if (u == u_begin) bseg_first = h0 + j0;
+                    if (it == 0) bseg_first = h0 + j0;
                     bseg_len += ui.nblk;
                 }
                 sm.info[s] = ui;
@@ -351,19 +323,16 @@ __global__ void __launch_bounds__(CWH_THREADS, CWH_MIN_CTAS) hash_kernel(const H
                 bulk_g2s(smem_u32(&sm.stage[s][0]), src, bytes, bar, policy);
                 // advance
                 ++t;
-                if (uo0 + t == uo1 && u + 1 < u_end) {
+                if (t == un && it + 1 < n_units) {
                     in_bseg = false;
-                    do {
-                        ++r;
-                        uo0 = uo1;
-                        uo1 = uo(r + 1);
-                    } while (uo1 == uo0);  // requests without work
+                    do ++r;
+                    while (req_info(a, r).units == 0);  // requests without work (n_units says one with work follows)
                     t = 0;
                     fresh = true;
                 }
             }
             // hand-over record (rec_tail_state is written by the consumers)
-            const bool tail_open = (uo0 + t) < uo1;  // the last request continues in the next range
+            const bool tail_open = t < un;  // the last request continues in the next range
             sm.rec_bseg_first = bseg_first;
             sm.rec_bseg_len = (u32)bseg_len;
             sm.rec_flags = (starts_mid ? CWH_REC_MID : 0u) | (in_bseg ? CWH_REC_TAIL_IS_BSEG : 0u) |
@@ -554,17 +523,11 @@ int32_t cwi_hash_blocks(cw_ctx* ctx, const i32* d_tokens, const u64* d_tok_off, 
     a.salt = d_salt;
     a.hash_off = d_hash_off;
     a.hashes = d_hashes;
-    a.unit_off = ctx->hash_unit_off;
     a.plan = ctx->hash_plan;
     a.rec = ctx->hash_rec;
     a.status = ctx->d_status;
     a.max_hashed = ctx->cfg.max_hashed_blocks;
     a.R = R;
-    a.small = R <= CWH_SMALL_R ? 1u : 0u;
-    if (!a.small) {
-        hash_plan_kernel<<<1, 1024, 0, ctx->s_main>>>(a);
-        CW_LAUNCH_CHECK(ctx);
-    }
     // never more CTAs than units could exist; small calls stay small
     u64 max_units = (ctx->cfg.max_hashed_blocks >> CWH_UNIT_LOG2) + R;
     int grid = (int)((u64)ctx->hash_grid < max_units ? (u64)ctx->hash_grid : max_units);
@@ -575,11 +538,11 @@ int32_t cwi_hash_blocks(cw_ctx* ctx, const i32* d_tokens, const u64* d_tok_off, 
 }
 
 // ------------------------------------------------------------------------------------- no-allocation entry point
-// cw_hash_blocks_static: the same two kernels, for callers that can create no cw_ctx because they may not call
+// cw_hash_blocks_static: the same kernel, for callers that can create no cw_ctx because they may not call
 // cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).  The scratch the ctx
-// would own — unit_off[R+1], the plan words, one hand-over record per CTA, a status word — lives in ONE file-scope
-// device array of fixed size (CWH_STATIC_BYTES, about 164 KiB), held by every GPU that loads the library until the
-// process exits.  Limits: R <= CW_HASH_STATIC_MAX_REQUESTS; any number of blocks.
+// would own — the plan words, one hand-over record per CTA, a status word — lives in ONE file-scope device array of
+// fixed size (CWH_STATIC_BYTES, about 32 KiB), held by every GPU that loads the library until the process exits.
+// Limits: R <= CW_HASH_STATIC_MAX_REQUESTS (the stated maximum of this entry point); any number of blocks.
 //
 // Host code must not hand `g_hash_static` itself to a kernel: in host code that name is a host-side stand-in, not a
 // device address.  The device address is fetched once per device with cudaGetSymbolAddress (that device current) and
@@ -587,8 +550,8 @@ int32_t cwi_hash_blocks(cw_ctx* ctx, const i32* d_tokens, const u64* d_tok_off, 
 //
 // Every call shares the array and it keeps the last call's contents.  What must start at zero — the range ticket and
 // the CTAs-done counter — is cleared at the start of every call (cudaMemsetAsync on the caller's stream: no
-// allocation); the epoch word deliberately persists (records of earlier calls go stale by epoch); unit_off and the
-// records are rewritten before they are read.  Two calls that overlap on the GPU (different streams, or graph branches)
+// allocation); the epoch word deliberately persists (records of earlier calls go stale by epoch); the records are
+// rewritten before they are read.  Two calls that overlap on the GPU (different streams, or graph branches)
 // RACE on the array: the caller serialises them.
 namespace {
 
@@ -596,14 +559,13 @@ constexpr u32 CWH_STATIC_MAX_R = 16384;    // == CW_HASH_STATIC_MAX_REQUESTS in 
 constexpr u32 CWH_STATIC_MAX_GRID = 2048;  // hand-over records (the grid is clamped to this)
 
 struct HashStaticScratch {
-    u64 unit_off[CWH_STATIC_MAX_R + 1];
-    u64 plan[4];  // [0] total units, [1] call epoch, [2] range ticket, [3] CTAs done
+    u64 plan[4];  // [1] call epoch, [2] range ticket, [3] CTAs done
     cw_hash_rec rec[CWH_STATIC_MAX_GRID];
     u32 status;   // device-detected conditions when the caller passes no d_status
     u32 pad[3];
 };
 constexpr size_t CWH_STATIC_BYTES = sizeof(HashStaticScratch);
-static_assert(CWH_STATIC_BYTES <= (192u << 10), "the static scratch is meant to stay modest");
+static_assert(CWH_STATIC_BYTES <= (64u << 10), "the static scratch is meant to stay modest");
 
 static __device__ __align__(256) unsigned char g_hash_static[CWH_STATIC_BYTES];
 
@@ -678,18 +640,12 @@ int32_t cw_hash_blocks_static(const int32_t* d_tokens, const uint64_t* d_tok_off
     a.salt = d_salt;
     a.hash_off = d_hash_off;
     a.hashes = d_hashes;
-    a.unit_off = reinterpret_cast<u64*>(reinterpret_cast<unsigned char*>(sc) + offsetof(HashStaticScratch, unit_off));
     a.plan = reinterpret_cast<u64*>(reinterpret_cast<unsigned char*>(sc) + offsetof(HashStaticScratch, plan));
     a.rec = reinterpret_cast<cw_hash_rec*>(reinterpret_cast<unsigned char*>(sc) + offsetof(HashStaticScratch, rec));
     a.status = d_status ? d_status
                         : reinterpret_cast<u32*>(reinterpret_cast<unsigned char*>(sc) + offsetof(HashStaticScratch, status));
     a.max_hashed = max_hashed_blocks;
     a.R = R;
-    a.small = R <= CWH_SMALL_R ? 1u : 0u;
-    if (!a.small) {
-        hash_plan_kernel<<<1, 1024, 0, s>>>(a);
-        if (cudaGetLastError() != cudaSuccess) return CW_E_CUDA;
-    }
     const u64 max_units = (max_hashed_blocks >> CWH_UNIT_LOG2) + R;
     int grid = (int)((u64)sd->grid < max_units ? (u64)sd->grid : max_units);
     if (grid < 1) grid = 1;

@@ -63,7 +63,6 @@ __host__ __device__ __forceinline__ u64 cw_remap_key(u64 k) {
 #define CWH_K 8                       // consecutive blocks a consumer lane owns inside a unit
 #define CWH_UNIT (32 * CWH_K)         // blocks per unit (one unit = one TMA copy = one consumer-warp iteration)
 #define CWH_UNIT_LOG2 8
-#define CWH_SMALL_R 512                // calls with at most this many requests skip the plan kernel
 #define CWH_STAGES 4                  // smem ring depth
 #define CWH_MIN_CTAS 3
 #define CWH_THREADS (32 * (CWH_WARPS + 1))
@@ -133,7 +132,6 @@ struct cw_ctx {
     u32* d_status;
     u32* h_status;  // pinned
     // stage 1
-    u64* hash_unit_off;  // max_requests + 1
     u64* hash_plan;
     cw_hash_rec* hash_rec;  // hash_grid
     int hash_grid;

@@ -123,9 +123,9 @@ def test_host_side_argument_checks(ctx):
 
 
 def test_small_and_large_calls_interleaved_on_one_context():
-    """Calls of at most 512 requests rebuild the plan inside the hash kernel (no plan kernel) and re-arm the range
-    ticket and the epoch themselves; larger calls go through the plan kernel.  Any order of the two on one context,
-    including long requests that span many ranges (look-back over dependent ranges), must stay bit-exact."""
+    """Every call cuts its own token space into ranges (no plan pass) and its last CTA re-arms the range ticket and
+    advances the epoch.  Small and large calls in any order on one context, including long requests that span many
+    ranges (look-back over dependent ranges), must stay bit-exact."""
     from gpu_util import small_ctx
     ctx = small_ctx(max_requests=4096, max_hashed_blocks=1 << 21)
     g = gen.rng(41, 0)

@@ -30,8 +30,8 @@ def test_static_scratch_hash_equals_the_ctx_path_on_two_calls_in_a_row():
     from gpu_util import dev, gpu_hash, hash_off_of, host, small_ctx, zeros
 
     g = gen.rng(97, 0)
-    # a large call (plan kernel, long request spanning ranges), then at once a small one (plan folded into the hash
-    # kernel; the scratch still holds the first call's offsets, records and epoch), then the large shape again
+    # a large call (long request spanning many ranges), then at once a small one (few ranges, most of the grid idle;
+    # the scratch still holds the first call's records and epoch), then a mid-sized one
     cases = [_queue(g, 3000, 300_000), _queue(g, 37, 70_000), _queue(g, 600, 0)]
     bufs = []
     for tokens, tok_off, salt in cases:                  # every caller-side buffer exists before the first call

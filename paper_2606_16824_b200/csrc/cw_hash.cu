@@ -217,9 +217,8 @@ __global__ void __launch_bounds__(CWH_THREADS, CWH_MIN_CTAS) hash_kernel(const H
     {   // every request's offsets are checked once, spread over the grid (the status word is all this produces)
         bool bad = too_big;
         for (u32 r = blockIdx.x * CWH_THREADS + tid; r < R; r += G * CWH_THREADS) bad |= req_info(a, r).invalid;
-        if (bad) atomicOr(a.status, CWS_INVAL);
+        if (__syncthreads_or(bad) && tid == 0) atomicOr(a.status, CWS_INVAL);  // (also makes sm.range visible)
     }
-    __syncthreads();
     auto call_done = [&]() {  // self-cleaning: the last CTA to finish re-arms the ticket and advances the epoch
         if (tid == 0) {
             const u32 old = atomicAdd(reinterpret_cast<unsigned int*>(a.plan + 3), 1u);

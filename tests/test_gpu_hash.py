@@ -87,6 +87,39 @@ def test_resume_from_start_block(ctx):
             assert (got[lo + sb[r]:int(ho[r + 1])] == cold[lo + sb[r]:int(ho[r + 1])]).all()
 
 
+def test_token_space_ranges_with_stretches_that_hold_no_work():
+    """The ranges are cut in TOKEN space and moved to unit boundaries: long stretches of tokens without any unit
+    (thousands of requests shorter than a block, requests resumed close to their end) leave ranges empty in the middle
+    of the grid, a range start may hop over many requests, and a long request behind them still spans many ranges."""
+    from gpu_util import small_ctx
+    ctx = small_ctx(max_requests=12000, max_hashed_blocks=1 << 21)
+    g = gen.rng(57, 0)
+    lens = np.concatenate([g.integers(0, 16, size=4000),                 # no full block at all
+                           [16 * 70_000 + 5],                            # one request over hundreds of ranges
+                           g.integers(0, 16, size=3000),
+                           g.integers(16 * 200, 16 * 3000, size=40),     # resumed close to their end below
+                           g.integers(0, 40, size=2000),
+                           [16 * 256 * 3, 16 * 256 * 3 + 1, 15, 16]]).astype(np.int64)
+    R = lens.size
+    tok_off = np.concatenate([[0], np.cumsum(lens)]).astype(np.uint64)
+    tokens = g.integers(0, gen.VOCAB, size=int(tok_off[-1]), dtype=np.int32)
+    salt = g.integers(0, 1 << 63, size=R, dtype=np.uint64)
+    cold, ho = oracle.hash_blocks(tokens, tok_off, salt=salt)
+    _check(ctx, tokens, tok_off, salt=salt)
+    n = (ho[1:] - ho[:-1]).astype(np.int64)
+    sb = np.zeros(R, np.int64)
+    sb[7001:7041] = np.maximum(n[7001:7041] - g.integers(0, 3, size=40), 0)     # 0..2 blocks left to hash
+    sb[4000] = 69_000
+    state = np.array([cold[int(ho[r]) + int(sb[r]) - 1] if sb[r] else 0 for r in range(R)], np.uint64)
+    init = np.full(cold.size, 0x2222222222222222, np.uint64)
+    got = _check(ctx, tokens, tok_off, salt=salt, start_block=sb.astype(np.uint32), start_state=state, hashes=init)
+    for r in (4000, 7001, 7020, 7040):
+        lo = int(ho[r])
+        assert (got[lo:lo + int(sb[r])] == 0x2222222222222222).all()
+        assert (got[lo + int(sb[r]):int(ho[r + 1])] == cold[lo + int(sb[r]):int(ho[r + 1])]).all()
+    ctx.close()
+
+
 def test_scaled_stress_queue_and_repeatability(ctx):
     snap = gen.stress_snapshot(seed=5, S=8, L=32768, RB=1024, req_per_session=16, len_median=4096, len_min=64,
                                len_max=32768)

@@ -497,7 +497,9 @@ def run_cuda(args):
             rooflines[name] = {"bound": "hbm", "achieved": round(ach, 1), "peak": hbm_peak, "unit": "GB/s",
                                "frac": round(ach / hbm_peak, 4), "traffic": traffic.get(name) if args.scale <= 1 else None,
                                "algorithmic_bytes": alg[name], "us": round(stage_ms[name] * 1e3, 2)}
-            if name in kern_us and name != "score_evict":   # the captured evict launch is the 37-CTA speculative one
+            # not for score_evict (the captured launch is the reduced speculative grid) nor for match (the call is
+            # three kernels: the probe kernel alone does not do the stage's work)
+            if name in kern_us and name not in ("score_evict", "match"):
                 rooflines[name]["main_kernel_alone_us_ncu"] = kern_us[name]
                 rooflines[name]["main_kernel_alone_frac_ncu"] = round(alg[name] / kern_us[name] / 1e3 / hbm_peak, 4)
     dominant = max(stage_ms, key=stage_ms.get)

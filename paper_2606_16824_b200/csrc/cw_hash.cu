@@ -11,15 +11,15 @@
 //   CTA  : the 4 consumer warps take the units of the CTA's range round-robin; the chain state is handed from the
 //          warp of unit i to the warp of unit i+1 through a shared-memory ring (one mbarrier per slot): the serial
 //          part per unit is one multiply-add, everything else of a unit runs beside the other warps' units
-//   grid : the list of units (request-aligned runs of <= 256 blocks) is cut into gridDim.x CONTIGUOUS ranges
-//          of about equal length (equal in tokens), one per CTA.  A CTA therefore walks its requests sequentially and never waits on
-//          another CTA (no look-back, no spinning).  Only the first request of a range can have begun in an
-//          earlier range: that boundary segment is scanned with carry-in 0 and patched at the very end of the
-//          CTA, H_j += A^(j-j0+1) * carry_in (linear in the carry, mod 2^64), from the chain states the CTAs of the
-//          earlier ranges have published (a range wholly inside one request publishes its carry-free tail and
-//          its length, and the reader folds those while walking back).  Ranges are handed out by an atomic ticket, so the
-//          CTA that is waited for has always started: the single wait per CTA cannot deadlock and happens
-//          when both CTAs are finishing anyway.
+//   grid : the list of units (request-aligned runs of <= 256 blocks) is cut into gridDim.x CONTIGUOUS ranges of
+//          about equal length (equal in tokens), one per CTA.  A CTA therefore walks its requests sequentially and
+//          never waits on another CTA while it streams.  Only the first request of a range can have begun in an
+//          earlier range: that boundary segment is scanned with carry-in 0 and patched at the very end of the CTA,
+//          H_j += A^(j-j0+1) * carry_in (linear in the carry, mod 2^64), from the chain states the CTAs of the
+//          earlier ranges have published (a range wholly inside one request publishes its carry-free tail and its
+//          length, and the reader folds those while walking back).  Ranges are handed out by an atomic ticket, so
+//          the CTA that is waited for has always started: the single wait per CTA cannot deadlock and happens when
+//          both CTAs are finishing anyway.
 //
 // One launch per call, no plan pass: the TOKEN space of the call is cut into gridDim.x equal pieces (a multiple of a
 // unit's 4096 tokens each) and every CTA moves the two ends of its piece to the first unit at or behind them by a
@@ -27,13 +27,12 @@
 // tile the unit list); the offsets of every request are validated once, spread over the grid; the last CTA to finish
 // re-arms the ticket and advances the epoch.  (Rounds 1-2 ran a one-CTA plan kernel first — units per request,
 // exclusive scan, 10 us plus a launch gap in front of an 87 us kernel — and cut the UNIT list into equal ranges.)
-//   hash_kernel        the streaming pass: one producer warp issues ONE TMA bulk copy (cp.async.bulk, L2
-//                      evict-first) of each unit's 16 KiB of token ids into a 4-stage shared-memory ring
-//                      (mbarrier full/empty); a consumer warp reads its unit with conflict-free 16-byte loads (the
-//                      quarter of a block a lane reads first is rotated by the lane id and odd lane quads take
-//                      their block pairs in swapped order, so the 8 lanes of a load phase cover all 32 banks);
-//                      16 multiplies + fin per block, the lane chain, the warp scan, the hand-over, 8 stores;
-//                      then the boundary patch (about half a request per CTA: ~1% extra traffic, L2-resident)
+// The streaming pass: one producer warp issues ONE TMA bulk copy (cp.async.bulk, L2 evict-first) of each unit's
+// 16 KiB of token ids into a 4-stage shared-memory ring (mbarrier full/empty); a consumer warp reads its unit with
+// conflict-free 16-byte loads (the quarter of a block a lane reads first is rotated by the lane id and odd lane quads
+// take their block pairs in swapped order, so the 8 lanes of a load phase cover all 32 banks); 16 multiplies + fin per
+// block, the lane chain, the warp scan, the hand-over, 8 stores; then the boundary patch (about half a request per
+// CTA: ~1% extra traffic, L2-resident).
 // Requests start at arbitrary 4-byte alignment: the copy starts at the 16-byte boundary below and the
 // consumers funnel the `mis` leading words away in registers.
 #include <stddef.h>
